@@ -1,0 +1,24 @@
+"""ORACLE -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+A plain, slow, obviously-correct fp64 (numpy) CPU implementation of what the
+mmx hot path computes: the finite-difference effective field, the
+Landau-Lifshitz-Gilbert right-hand side and its Runge-Kutta advance, written
+from /root/reference/PAPER.md (cited as P:L<line>) with the readings listed in
+DESIGN.md ("S-list") wherever the paper is silent.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline /
+`--impl reference` legs may import this package.  It shares no code with
+`paper_2411_18194_b200/` (the CUDA path); only the seeded input generators in
+`workloads/` serve both sides.
+
+Pin status (see tests/test_oracle_*.py and DESIGN.md section "Oracle pins"):
+  newell / demag .......... pinned (P1-P5, P19, mpmath spot values, dipole limit)
+  exchange, DMI, anisotropy pinned (P6, P10, P11)
+  sublattice exchange ..... pinned (P10, P12)
+  LLG torque, integrators . pinned (P7, P8, P9, P14)
+  Zhang-Li torque ......... pinned (P13: Gilbert-form identity, rigid translation at -u)
+  elastic / magnetoelastic  pinned (P15 paper numbers, P16 patch test, P17)
+  adaptive-step controller constants (S21), PBC image window (S13), which
+  config switches c3 uses (S8, S14): parity unpinned -- definitions shared by
+  both sides, stated in DESIGN.md.
+"""

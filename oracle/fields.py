@@ -1,0 +1,183 @@
+"""ORACLE (test infrastructure): local effective-field terms and torques.
+
+All arrays are float64, vector fields are [3, Nz, Ny, Nx] (component first),
+per-cell scalars [Nz, Ny, Nx].  Axis numbering: 0 = x, 1 = y, 2 = z.
+
+Citations: exchange Eq.3; DMI Eq.4; anisotropy / Zeeman
+P:L116-118 ("implemented in the same way as in mumax3" -- readings S3, S16);
+magnetoelastic field Eq.9; LLG torque Eq.2; Zhang-Li
+torque P:L110 (reading S17).  Boundary reading S9 (OPEN = a stencil pair whose
+partner does not exist contributes nothing).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from .constants import MU_B, Q_E
+
+
+# ----------------------------------------------------------------------
+# neighbour access
+# ----------------------------------------------------------------------
+def neighbour(a, axis, d, periodic):
+    """Value of `a` at cell c + d*e_axis, and whether that cell is inside the grid
+    (after wrapping on a periodic axis).  Outside cells read as 0."""
+    ax = a.ndim - 1 - axis
+    n = a.shape[ax]
+    if periodic:
+        return np.roll(a, -d, axis=ax), np.ones(a.shape[-3:], dtype=bool)
+    out = np.zeros_like(a)
+    ex = np.zeros(a.shape[-3:], dtype=bool)
+    if abs(d) < n:
+        src = [slice(None)] * a.ndim
+        dst = [slice(None)] * a.ndim
+        if d > 0:
+            dst[ax], src[ax] = slice(0, n - d), slice(d, n)
+        else:
+            dst[ax], src[ax] = slice(-d, n), slice(0, n + d)
+        out[tuple(dst)] = a[tuple(src)]
+        exd = [slice(None)] * 3
+        exd[2 - axis] = dst[ax]
+        ex[tuple(exd)] = True
+    return out, ex
+
+
+def _harmonic(a, b):
+    s = a + b
+    out = np.zeros_like(s)
+    np.divide(2 * a * b, s, out=out, where=(s != 0))
+    return out
+
+
+def _inv(ms):
+    out = np.zeros_like(ms)
+    np.divide(1.0, ms, out=out, where=(ms > 0))
+    return out
+
+
+# ----------------------------------------------------------------------
+# Eq.3: exchange-like pair terms
+# ----------------------------------------------------------------------
+def pair_laplacian(mq, Ms, Apar, reg, scale, cell, pbc, factor):
+    """sum over the 6 neighbours n of  factor * A_cn / Ms_c * (mq_n - mq_c) / h_n^2,
+    A_cn = harmonic mean of Apar at c and n, times `scale` when c and n lie in
+    different regions (S3, S4).  factor=2, mq=m^(s), Apar=A11: first term of Eq.3;
+    factor=1, mq=m^(s'), Apar=A12: second term (S5)."""
+    B = np.zeros_like(mq)
+    iMs = _inv(Ms)
+    for axis in range(3):
+        h = cell[axis]
+        for d in (+1, -1):
+            mn, ex = neighbour(mq, axis, d, pbc[axis] > 0)
+            Msn, _ = neighbour(Ms, axis, d, pbc[axis] > 0)
+            An, _ = neighbour(Apar, axis, d, pbc[axis] > 0)
+            rn, _ = neighbour(reg, axis, d, pbc[axis] > 0)
+            ok = ex & (Msn > 0) & (Ms > 0)
+            Acn = _harmonic(Apar, An) * np.where(rn == reg, 1.0, scale)
+            B += np.where(ok, factor * Acn * iMs / (h * h), 0.0)[None] * (mn - mq)
+    return B
+
+
+def homogeneous_exchange(m_other, Ms, A0, latcon):
+    """Third term of Eq.3: 4 A0 / (Ms a^2) m^(s')."""
+    return (4.0 * A0 / (latcon * latcon)) * _inv(Ms)[None] * m_other
+
+
+# ----------------------------------------------------------------------
+# Eq.4, interfacial subset (S7): D_xzx = D_yzy = +D, D_xxz = D_yyz = -D
+# ----------------------------------------------------------------------
+def dmi_interfacial(mq, Ms, D, cell, pbc):
+    """B = sum_{n in +-x, +-y} D_cn / (Ms_c h_n) (z^ x e_cn) x mq_n ;
+    continuum limit (2D/Ms)(dx m_z, dy m_z, -dx m_x - dy m_y)."""
+    B = np.zeros_like(mq)
+    iMs = _inv(Ms)
+    for axis in (0, 1):
+        h = cell[axis]
+        for d in (+1, -1):
+            mn, ex = neighbour(mq, axis, d, pbc[axis] > 0)
+            Msn, _ = neighbour(Ms, axis, d, pbc[axis] > 0)
+            Dn, _ = neighbour(D, axis, d, pbc[axis] > 0)
+            ok = ex & (Msn > 0) & (Ms > 0)
+            w = np.where(ok, _harmonic(D, Dn) * iMs / h, 0.0) * d
+            # (z^ x (d x^)) x m = d ( m_z, 0, -m_x);  (z^ x (d y^)) x m = d (0, m_z, -m_y)
+            B[axis] += w * mn[2]
+            B[2] -= w * mn[axis]
+    return B
+
+
+# ----------------------------------------------------------------------
+# anisotropy, Zeeman (S16)
+# ----------------------------------------------------------------------
+def uniaxial(m, Ms, Ku1, u):
+    """B = (2 Ku1 / Ms) (u.m) u ; u [3,Nz,Ny,Nx] unit axis per cell."""
+    return (2.0 * Ku1 * _inv(Ms) * (u * m).sum(axis=0))[None] * u
+
+
+def cubic(m, Ms, Kc1, c1, c2):
+    """B = -(2 Kc1/Ms) sum_i (c_i.m) [ (c_j.m)^2 + (c_k.m)^2 ] c_i, c3 = c1 x c2."""
+    c3 = np.cross(c1, c2, axis=0)
+    a = [(c * m).sum(axis=0) for c in (c1, c2, c3)]
+    pref = -2.0 * Kc1 * _inv(Ms)
+    B = np.zeros_like(m)
+    for i, c in enumerate((c1, c2, c3)):
+        j, k = (i + 1) % 3, (i + 2) % 3
+        B += (pref * a[i] * (a[j] ** 2 + a[k] ** 2))[None] * c
+    return B
+
+
+def zeeman(m, Ms, bext):
+    return np.asarray(bext, float)[:, None, None, None] * (Ms > 0)[None] * np.ones_like(m)
+
+
+# ----------------------------------------------------------------------
+# Eq.9: magnetoelastic (Villari) field; eps = dict xx,yy,zz,xy,xz,yz of tensor strain
+# ----------------------------------------------------------------------
+def magnetoelastic_field(m, Ms, B1, B2, eps):
+    pref = -2.0 * _inv(Ms)
+    out = np.empty_like(m)
+    out[0] = pref * (B1 * eps["xx"] * m[0] + B2 * (eps["xy"] * m[1] + eps["xz"] * m[2]))
+    out[1] = pref * (B1 * eps["yy"] * m[1] + B2 * (eps["xy"] * m[0] + eps["yz"] * m[2]))
+    out[2] = pref * (B1 * eps["zz"] * m[2] + B2 * (eps["xz"] * m[0] + eps["yz"] * m[1]))
+    return out
+
+
+# ----------------------------------------------------------------------
+# torques
+# ----------------------------------------------------------------------
+def cross(a, b):
+    return np.stack([a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]])
+
+
+def llg_torque(m, B, alpha, gamma):
+    """Eq.2: tau = -gamma/(1+alpha^2) [ m x B + alpha m x (m x B) ]   (1/s)."""
+    mxB = cross(m, B)
+    return (-gamma / (1.0 + alpha * alpha))[None] * (mxB + alpha[None] * cross(m, mxB))
+
+
+def directional_derivative(m, uvec, Ms, cell, pbc):
+    """(u.grad) m by 2-point central differences; a missing neighbour takes the
+    centre value (S17).  uvec [3,Nz,Ny,Nx] in m/s."""
+    out = np.zeros_like(m)
+    for axis in range(3):
+        h = cell[axis]
+        per = pbc[axis] > 0
+        mp, exp_ = neighbour(m, axis, +1, per)
+        mm, exm = neighbour(m, axis, -1, per)
+        Mp, _ = neighbour(Ms, axis, +1, per)
+        Mm, _ = neighbour(Ms, axis, -1, per)
+        mp = np.where((exp_ & (Mp > 0))[None], mp, m)
+        mm = np.where((exm & (Mm > 0))[None], mm, m)
+        out += uvec[axis][None] * (mp - mm) / (2.0 * h)
+    return out
+
+
+def zhang_li_torque(m, Ms, alpha, pol, xi, J, cell, pbc):
+    """tau_ZL = -(1+alpha^2)^-1 [ (1+xi alpha) m x (m x (u.grad)m) + (xi-alpha) m x (u.grad)m ],
+    u = mu_B P J / (e Ms (1+xi^2))  [m/s]   (S17; per sublattice with its own Ms, S18)."""
+    Jv = np.asarray(J, float)
+    uvec = (MU_B * pol * _inv(Ms) / (Q_E * (1.0 + xi * xi)))[None] * Jv[:, None, None, None]
+    a = directional_derivative(m, uvec, Ms, cell, pbc)
+    mxa = cross(m, a)
+    mxmxa = cross(m, mxa)
+    return (-1.0 / (1.0 + alpha * alpha))[None] * ((1.0 + xi * alpha)[None] * mxmxa
+                                                   + (xi - alpha)[None] * mxa)

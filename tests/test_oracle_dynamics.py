@@ -1,0 +1,184 @@
+"""Pins for the torque and the integrators of the oracle (P7, P8, P9, P12, P13, P14)."""
+from fractions import Fraction as Fr
+
+import numpy as np
+
+import workloads as wl
+from oracle import fields as fl
+from oracle import rk
+from oracle.constants import GAMMA, MU_B, Q_E, T_ALL
+from oracle.world import World
+
+
+def _macrospin(alpha, B=1.0, m0=(0.6, 0.0, 0.8)):
+    m = np.array(m0, np.float64).reshape(3, 1, 1, 1)
+    spec = wl.WorldSpec(name="macro", grid=(1, 1, 1), cell=(1e-9,) * 3, demag=False,
+                        mat=wl.make_mat(1, Ms=8e5, alpha=alpha), coupling=wl.default_coupling(),
+                        bext=(0, 0, B), m=[m.astype(np.float32)])
+    w = World(spec)
+    w.m = [m.copy()]  # exact double start
+    return w
+
+
+def _macrospin_exact(alpha, B, m0, t):
+    mz = np.tanh(alpha * GAMMA * B * t / (1 + alpha ** 2) + np.arctanh(m0[2]))
+    phi = np.arctan2(m0[1], m0[0]) + GAMMA * B * t / (1 + alpha ** 2)
+    s = np.sqrt(1 - mz * mz)
+    return np.array([s * np.cos(phi), s * np.sin(phi), mz])
+
+
+def test_P7_macrospin_precession_and_damping():
+    for alpha in (0.0, 0.02, 0.5):
+        w = _macrospin(alpha)
+        w.step_rk4(1e-13, 500)
+        want = _macrospin_exact(alpha, 1.0, (0.6, 0.0, 0.8), 500e-13)
+        np.testing.assert_allclose(w.m[0].ravel(), want, atol=2e-9)
+        assert abs(np.linalg.norm(w.m[0].ravel()) - 1) < 1e-15  # P8
+
+
+def test_P14_tableau_identities():
+    for tab in (rk.RK4, rk.DP45):
+        assert abs(sum(tab.b) - 1) < 1e-15
+        for i in range(tab.stages):
+            assert abs(sum(tab.a[i]) - tab.c[i]) < 1e-15
+    # e = b - b*, b* the embedded 4th-order weights of the Dormand-Prince pair (ref [55])
+    bstar = [Fr(5179, 57600), 0, Fr(7571, 16695), Fr(393, 640), Fr(-92097, 339200), Fr(187, 2100), Fr(1, 40)]
+    for bj, bs, ej in zip(rk.DP45.b, bstar, rk.DP45.e):
+        assert abs((bj - float(bs)) - ej) < 1e-16
+    # order conditions: b up to order 5 (bushy + a few tall trees), b* up to order 4
+    a = np.zeros((7, 7))
+    for i, row in enumerate(rk.DP45.a):
+        a[i, :len(row)] = row
+    c = np.array(rk.DP45.c)
+    for wts, order in ((np.array(rk.DP45.b), 5), (np.array([float(x) for x in bstar]), 4)):
+        for k in range(order):
+            assert abs(wts @ c ** k - 1 / (k + 1)) < 1e-14
+        assert abs(wts @ (a @ c) - 1 / 6) < 1e-14
+        assert abs(wts @ (a @ c ** 2) - 1 / 12) < 1e-14
+        assert abs(wts @ (a @ (a @ c)) - 1 / 24) < 1e-14
+        assert abs(wts @ (c * (a @ c)) - 1 / 8) < 1e-14
+    b5 = np.array(rk.DP45.b)
+    assert abs(b5 @ (a @ c ** 3) - 1 / 20) < 1e-14
+    assert abs(b5 @ (a @ (a @ (a @ c))) - 1 / 120) < 1e-14
+    # FSAL: last row of a equals b
+    np.testing.assert_allclose(rk.DP45.a[6], rk.DP45.b[:6])
+
+
+def _final_error(method, dt, T=2e-11, alpha=0.3):
+    w = _macrospin(alpha, B=2.0)
+    n = int(round(T / dt))
+    if method == "rk4":
+        w.step_rk4(dt, n)
+    else:
+        w.step_dp45_fixed(dt, n)
+    return np.abs(w.m[0].ravel() - _macrospin_exact(alpha, 2.0, (0.6, 0.0, 0.8), n * dt)).max()
+
+
+def test_P14_observed_orders():
+    """Table 2: Dormand-Prince convergence order 5, error-estimate order 4; RK4 order 4."""
+    e1, e2 = _final_error("rk4", 1e-12), _final_error("rk4", 0.5e-12)
+    assert 3.7 < np.log2(e1 / e2) < 4.4
+    e1, e2 = _final_error("dp45", 1e-12), _final_error("dp45", 0.5e-12)
+    assert 4.6 < np.log2(e1 / e2) < 5.5
+    # local error estimate ~ dt^5 (a 4th-order embedded solution)
+    est = []
+    for dt in (1e-12, 0.5e-12):
+        w = _macrospin(0.3, B=2.0)
+        est.append(w.step_dp45_fixed(dt, 1)[0])
+    assert 4.6 < np.log2(est[0] / est[1]) < 5.4
+
+
+def _small_world(alpha, seed=21, S=1, J=(0, 0, 0)):
+    rng = np.random.default_rng(seed)
+    grid = (6, 4, 2)
+    spec = wl.WorldSpec(
+        name="small", grid=grid, cell=(3e-9, 3e-9, 2e-9), S=S,
+        mat=wl.make_mat(S, Ms=8e5, A=1.3e-11, alpha=alpha, Ku1=5e4, D=1e-3, Kc1=2e4),
+        coupling=wl.default_coupling(A0=-4e-15, A12=-1e-12, D_inter=3e-4), bext=(0.0, 0.01, 0.05), J=J,
+        m=[wl.smoothed_random_unit(rng, grid, 2.0) for _ in range(S)])
+    return World(spec, demag_mode="direct")
+
+
+def test_P9_energy_conservation_and_dissipation():
+    """alpha = 0: total energy constant to integrator order.  alpha > 0:
+    dE/dt = -alpha gamma/(1+alpha^2) sum Ms V |m x B|^2."""
+    drift = []
+    for dt in (4e-14, 2e-14):
+        w = _small_world(0.0, S=2)
+        E0 = w.energy()
+        w.step_rk4(dt, int(round(8e-13 / dt)))
+        drift.append(abs(w.energy() - E0) / abs(E0))
+    assert drift[0] < 1e-6 and drift[1] < drift[0] / 8
+    alpha = 0.2
+    w = _small_world(alpha, S=2)
+    rate = 0.0
+    for s in range(2):
+        mxB = fl.cross(w.m[s], w.heff(s))
+        rate += -alpha * GAMMA / (1 + alpha ** 2) * float((w.p[s]["Ms"][None] * mxB ** 2).sum()) * w.V
+    E0 = w.energy()
+    dt = 1e-15
+    w.step_rk4(dt, 1)
+    E1 = w.energy()
+    w.step_rk4(dt, 1)
+    E2 = w.energy()
+    num = (-3 * E0 + 4 * E1 - E2) / (2 * dt)
+    assert rate < 0 and abs(num - rate) < 1e-4 * abs(rate)
+
+
+def test_P12_antiferromagnetic_resonance():
+    """Two antiparallel macrospins, small tilt: omega = gamma sqrt(B_A (2 B_E + B_A)),
+    B_E = -4 A0/(Ms a^2), B_A = 2 Ku/Ms  -> 128.3 GHz for the c3 numbers."""
+    Ms, A0, a, Ku = 4.0e5, -4.0e-13, 0.35e-9, 6.4e4
+    BE, BA = -4 * A0 / (Ms * a * a), 2 * Ku / Ms
+    f_want = GAMMA * np.sqrt(BA * (2 * BE + BA)) / (2 * np.pi)
+    assert abs(f_want - 128.3e9) < 0.1e9
+    m1 = np.array([1e-4, 0, 1.0]).reshape(3, 1, 1, 1)
+    m2 = np.array([0, 0, -1.0]).reshape(3, 1, 1, 1)
+    spec = wl.WorldSpec(name="afmr", grid=(1, 1, 1), cell=(2e-9,) * 3, S=2, demag=False,
+                        mat=wl.make_mat(2, Ms=Ms, Ku1=Ku, alpha=0.0),
+                        coupling=wl.default_coupling(A0=A0, latcon=a),
+                        m=[m1.astype(np.float32), m2.astype(np.float32)])
+    w = World(spec)
+    w.m = [m1 / np.linalg.norm(m1), m2.copy()]
+    dt, n = 1e-14, 2400
+    xs = []
+    for _ in range(n):
+        w.step_dp45_fixed(dt, 1)
+        xs.append(w.m[0][0, 0, 0, 0] - w.m[1][0, 0, 0, 0] * 0)  # m1_x
+    xs = np.array(xs)
+    t = dt * np.arange(1, n + 1)
+    zc = np.nonzero(np.sign(xs[1:]) != np.sign(xs[:-1]))[0]
+    tz = t[zc] - xs[zc] * dt / (xs[zc + 1] - xs[zc])
+    # m1_x(t) = sum of the two degenerate circular modes: pure cos(omega t) -> half periods
+    f_got = 0.5 / np.mean(np.diff(tz))
+    assert abs(f_got - f_want) < 2e-3 * f_want
+
+
+def test_P13_zhang_li():
+    """alpha = xi: the Zhang-Li torque reduces to the transverse part of (u.grad)m, with
+    u = mu_B P j/(e Ms (1+xi^2)) (71.6 m/s for the c3 numbers); a wall translates rigidly at -u."""
+    Ms, P, xi, j = 4.0e5, 0.5, 0.1, 1e12
+    u = MU_B * P * j / (Q_E * Ms * (1 + xi * xi))
+    assert abs(u - 71.6) < 0.1
+    nx, h = 160, 2e-9
+    A, Ku = 1.0e-11, 6.4e4
+    spec = wl.WorldSpec(name="zl", grid=(nx, 1, 1), cell=(h, h, h), demag=False,
+                        mat=wl.make_mat(1, Ms=Ms, A=A, Ku1=Ku, alpha=xi, pol=P, xi=xi),
+                        coupling=wl.default_coupling(), J=(j, 0, 0),
+                        m=[wl.neel_wall((nx, 1, 1), (h, h, h), 0.5 * nx * h, np.sqrt(A / Ku))])
+    w = World(spec)
+    p = w.p[0]
+    tzl = fl.zhang_li_torque(w.m[0], p["Ms"], p["alpha"], p["pol"], p["xi"], w.J, w.cell, w.pbc)
+    a = fl.directional_derivative(w.m[0], np.array([u, 0, 0]).reshape(3, 1, 1, 1) * np.ones_like(w.m[0]),
+                                  p["Ms"], w.cell, w.pbc)
+    a_perp = a - (a * w.m[0]).sum(axis=0)[None] * w.m[0]
+    np.testing.assert_allclose(tzl, a_perp, atol=1e-9 * np.abs(a).max())
+    # dynamic: wall centre q from integral of m_z (m_z = tanh((x-q)/D)  =>  sum m_z h = L - 2q)
+    w.spec.J, w.J = (0, 0, 0), (0, 0, 0)
+    w.step_rk4(5e-14, 400)  # settle the analytic profile on the lattice (alpha = 0.1: partly)
+    w.J = (j, 0, 0)
+    q0 = 0.5 * (nx * h - w.m[0][2].sum() * h)
+    T = 4e-11
+    w.step_rk4(5e-14, int(round(T / 5e-14)))
+    q1 = 0.5 * (nx * h - w.m[0][2].sum() * h)
+    assert abs((q1 - q0) / T + u) < 0.02 * u

@@ -1,0 +1,138 @@
+"""Pins for oracle/fields.py and the energy bookkeeping of oracle/world.py (P6, P10, P11)."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import fields as fl
+from oracle.constants import (T_A0, T_A12, T_ANIS_C, T_ANIS_U, T_DEMAG, T_DMI, T_DMI_INTER, T_EXCH,
+                              T_MEL, T_ZEEMAN)
+from oracle.world import World
+
+
+def test_P6_exchange_spin_wave():
+    """m = (cos kx, sin kx, 0), periodic: B_exch = -(2A/Ms)(2/h^2)(1 - cos kh) m."""
+    nx, h, A, Ms = 32, 2e-9, 1.3e-11, 8e5
+    k = 2 * np.pi * 3 / (nx * h)
+    x = (np.arange(nx) + 0.5) * h
+    m = np.zeros((3, 1, 1, nx))
+    m[0, 0, 0], m[1, 0, 0] = np.cos(k * x), np.sin(k * x)
+    one = np.ones((1, 1, nx))
+    B = fl.pair_laplacian(m, Ms * one, A * one, np.zeros((1, 1, nx), int), 1.0, (h, h, h), (1, 0, 0), 2.0)
+    want = -(2 * A / Ms) * (2 / h ** 2) * (1 - np.cos(k * h)) * m
+    np.testing.assert_allclose(B, want, rtol=0, atol=1e-12 * np.abs(want).max())
+
+
+def test_P11_dmi_cycloid_and_continuum():
+    """m = (sin kx, 0, cos kx): B_DMI = -(2D/Ms)(sin kh / h) m; 2-D continuum limit
+    (2D/Ms)(dx mz, dy mz, -dx mx - dy my) for a smooth texture."""
+    nx, h, D, Ms = 40, 2e-9, 3e-3, 5.8e5
+    k = 2 * np.pi * 2 / (nx * h)
+    x = (np.arange(nx) + 0.5) * h
+    m = np.zeros((3, 1, 1, nx))
+    m[0, 0, 0], m[2, 0, 0] = np.sin(k * x), np.cos(k * x)
+    one = np.ones((1, 1, nx))
+    B = fl.dmi_interfacial(m, Ms * one, D * one, (h, h, h), (1, 0, 0))
+    want = -(2 * D / Ms) * (np.sin(k * h) / h) * m
+    np.testing.assert_allclose(B, want, rtol=0, atol=1e-12 * np.abs(want).max())
+    # 2-D smooth texture, periodic, checks the y-direction signs
+    n = 64
+    X, Y = np.meshgrid((np.arange(n) + 0.5) * h, (np.arange(n) + 0.5) * h, indexing="xy")
+    L = n * h
+    th = 0.3 * np.sin(2 * np.pi * X / L) + 0.2 * np.cos(2 * np.pi * Y / L) + 1.0
+    ph = 0.4 * np.sin(2 * np.pi * Y / L) + 0.1 * np.sin(2 * np.pi * X / L)
+    m = np.stack([np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph), np.cos(th)])[:, None]
+    one = np.ones((1, n, n))
+    B = fl.dmi_interfacial(m, Ms * one, D * one, (h, h, h), (1, 1, 0))
+
+    def d(f, ax):  # spectral derivative of a periodic array
+        kk = 2j * np.pi * np.fft.fftfreq(n, h)
+        shape = [1, 1, 1]
+        shape[ax] = n
+        return np.real(np.fft.ifft(np.fft.fft(f, axis=ax) * kk.reshape(shape), axis=ax))
+    want = (2 * D / Ms) * np.stack([d(m[2], 2), d(m[2], 1), -d(m[0], 2) - d(m[1], 1)])
+    assert np.abs(B - want).max() < 5e-3 * np.abs(want).max()  # O((kh)^2) stencil error
+
+
+def _toy_world(pbc, seed=3, elastic=False):
+    rng = np.random.default_rng(seed)
+    grid = (5, 4, 3)
+    S, R = 2, 3
+    mat = wl.make_mat(S, R,
+                      Ms=np.array([[4e5, 5e5, 3e5], [4.5e5, 3.5e5, 5.5e5]]),
+                      A=np.array([[1e-11, 0.7e-11, 1.3e-11], [0.9e-11, 1.1e-11, 0.8e-11]]),
+                      alpha=0.1, Ku1=np.array([[6e4, 3e4, 8e4], [5e4, 7e4, 2e4]]),
+                      Kc1=np.array([[1e4, -2e4, 3e4], [2e4, 1e4, -1e4]]),
+                      D=np.array([[1e-3, 2e-3, 0.5e-3], [1.5e-3, 1e-3, 2e-3]]),
+                      B1=-1e7, B2=-0.7e7)
+    ax = rng.standard_normal((S, R, 3))
+    mat["u"] = ax / np.linalg.norm(ax, axis=-1, keepdims=True)
+    c1 = rng.standard_normal((S, R, 3))
+    c1 /= np.linalg.norm(c1, axis=-1, keepdims=True)
+    c2 = np.cross(c1, rng.standard_normal((S, R, 3)))
+    c2 /= np.linalg.norm(c2, axis=-1, keepdims=True)
+    mat["c1"], mat["c2"] = c1, c2
+    spec = wl.WorldSpec(
+        name="toy", grid=grid, cell=(2e-9, 2.5e-9, 1.5e-9), pbc=pbc, S=S,
+        regions=rng.integers(0, R, (grid[2], grid[1], grid[0])).astype(np.uint16), mat=mat,
+        coupling=wl.default_coupling(A0=-4e-13, A12=-1e-12, D_inter=0.8e-3, scale_A11=0.25, scale_A12=0.5),
+        bext=(0.05, -0.02, 0.1),
+        elastic=dict(C11=2.5e11, C12=1.5e11, C44=1.0e11, rho=6800.0) if elastic else None,
+        m=[wl.random_unit(rng, grid), wl.random_unit(rng, grid)],
+        u=(rng.standard_normal((3, grid[2], grid[1], grid[0])) * 1e-12).astype(np.float32) if elastic else None,
+        v=np.zeros((3, grid[2], grid[1], grid[0]), np.float32) if elastic else None)
+    return World(spec, demag_mode="direct")
+
+
+@pytest.mark.parametrize("pbc", [(0, 0, 0), (1, 1, 0)])
+@pytest.mark.parametrize("term", [T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0,
+                                  T_DMI_INTER, T_MEL])
+def test_P10_field_is_energy_gradient(pbc, term):
+    """B_term = -(1/(Ms V)) dE_term/dm (unconstrained derivative of the oracle's energy),
+    including OPEN boundary pairs, region-pair scaling and two sublattices."""
+    w = _toy_world(pbc, elastic=True)
+    B = [w.heff(s, terms=term) for s in range(2)]
+    rng = np.random.default_rng(11)
+    scale = max(np.abs(B[0]).max(), np.abs(B[1]).max())
+    assert scale > 0
+    for _ in range(6):
+        s = int(rng.integers(0, 2))
+        c = int(rng.integers(0, 3))
+        iz, iy, ix = (int(rng.integers(0, n)) for n in (3, 4, 5))
+        m0 = w.m[s][c, iz, iy, ix]
+        hstep = 1e-4
+        E = []
+        for sgn in (+1, -1):
+            w.m[s][c, iz, iy, ix] = m0 + sgn * hstep
+            E.append(w.energy(term))
+        w.m[s][c, iz, iy, ix] = m0
+        dE = (E[0] - E[1]) / (2 * hstep)
+        want = -dE / (w.p[s]["Ms"][iz, iy, ix] * w.V)
+        assert abs(B[s][c, iz, iy, ix] - want) < 1e-6 * scale, (term, s, c)
+
+
+def test_open_boundary_pairs_contribute_nothing():
+    """S9: a uniform state has zero exchange field in every cell, also at open edges,
+    and the DMI field of a uniform state is an edge-only term."""
+    grid = (6, 5, 2)
+    one = np.ones((2, 5, 6))
+    m = np.zeros((3, 2, 5, 6))
+    m[0] = 0.6
+    m[2] = 0.8
+    B = fl.pair_laplacian(m, 8e5 * one, 1e-11 * one, np.zeros((2, 5, 6), int), 1.0, (1e-9,) * 3, (0, 0, 0), 2.0)
+    assert np.abs(B).max() == 0.0
+    Bd = fl.dmi_interfacial(m, 8e5 * one, 1e-3 * one, (1e-9,) * 3, (0, 0, 0))
+    assert np.abs(Bd[:, :, 1:-1, 1:-1]).max() < 1e-18
+    assert np.abs(Bd[:, :, :, 0]).max() > 0
+
+
+def test_anisotropy_special_cases():
+    one = np.ones((1, 1, 1))
+    m = np.array([0.6, 0.0, 0.8]).reshape(3, 1, 1, 1)
+    z = np.array([0.0, 0.0, 1.0]).reshape(3, 1, 1, 1)
+    x = np.array([1.0, 0.0, 0.0]).reshape(3, 1, 1, 1)
+    y = np.array([0.0, 1.0, 0.0]).reshape(3, 1, 1, 1)
+    Bu = fl.uniaxial(m, 8e5 * one, 5e5 * one, z)
+    np.testing.assert_allclose(Bu.ravel(), [0, 0, 2 * 5e5 / 8e5 * 0.8])
+    # cubic: B_x = -(2Kc1/Ms) m_x (m_y^2 + m_z^2)
+    Bc = fl.cubic(m, 8e5 * one, 1e4 * one, x, y)
+    np.testing.assert_allclose(Bc.ravel(), [-(2e4 / 8e5) * 0.6 * 0.64, 0, -(2e4 / 8e5) * 0.8 * 0.36], atol=1e-18)
