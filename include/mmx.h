@@ -1,0 +1,230 @@
+/* mmx.h -- C-ABI boundary of the B200-native micromagnetic hot path.
+ *
+ * The calls follow the statement of the problem in arxiv 2411.18194 (mumax+),
+ * cited as P:L<line> of PAPER.md: a simulation *world* holds one magnet
+ * with 1 or 2 sublattices; the magnet has per-region
+ * material parameters; the effective field (Eq.3, Eq.4, Eq.9, P:L116,
+ * P:L142-144) enters the LLG torque (Eq.2) which is advanced in
+ * time by an explicit / embedded Runge-Kutta method (Table 2),
+ * optionally together with the elastodynamic equation (Eq.7-8).
+ *
+ * Conventions
+ *   - plain C, no C++/torch types; every call returns an mmx_status (0 = OK),
+ *     never throws, never aborts.  mmx_last_error() gives the message of the
+ *     last failing call on this thread.
+ *   - units are SI: lengths m, fields T, Ms A/m, A J/m, K J/m^3, D J/m^2,
+ *     torque 1/s, current density A/m^2, time s.
+ *   - vector fields are fp32, structure-of-arrays [3][Nz][Ny][Nx], x fastest.
+ *   - pointers are tagged MMX_HOST or MMX_DEVICE by an explicit `mem` argument;
+ *     the caller owns every pointer it passes, the library never keeps it
+ *     after the call returns.  The world owns all of its device storage.
+ *   - all device work is enqueued on the CUDA stream given at creation
+ *     (NULL = legacy default stream).  Calls with host out-parameters
+ *     synchronise that stream; the others are asynchronous.
+ *   - there is no CPU fallback: without a CUDA device mmx_world_create fails
+ *     with MMX_ECUDA.
+ */
+#ifndef MMX_H
+#define MMX_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mmx_world mmx_world; /* opaque, library-owned */
+
+typedef enum {
+  MMX_OK = 0,
+  MMX_EINVAL = -1, /* bad argument (NULL, size, non power-of-two periodic axis ...) */
+  MMX_ENOMEM = -2, /* host or device allocation failed */
+  MMX_ECUDA = -3,  /* a CUDA runtime call or kernel failed; no device */
+  MMX_ESTATE = -4, /* call order (e.g. demag term requested before mmx_demag_kernel_init) */
+  MMX_ENAN = -5    /* NaN/Inf reached the error or torque reduction */
+} mmx_status;
+
+enum { MMX_HOST = 0, MMX_DEVICE = 1 };
+
+/* effective-field term bits for term_mask arguments */
+enum {
+  MMX_T_EXCH = 1,        /* Eq.3 first term: 2 A11/Ms lap m */
+  MMX_T_DMI = 2,         /* Eq.4 interfacial subset, same sublattice */
+  MMX_T_ANIS_U = 4,      /* uniaxial Ku1 */
+  MMX_T_ANIS_C = 8,      /* cubic Kc1     */
+  MMX_T_ZEEMAN = 16,     /* external field     */
+  MMX_T_DEMAG = 32,      /* magnetostatic field */
+  MMX_T_A12 = 64,        /* Eq.3 second term: A12/Ms lap m'                            */
+  MMX_T_A0 = 128,        /* Eq.3 third term: 4 A0/(a^2 Ms) m'                          */
+  MMX_T_DMI_INTER = 256, /* Eq.4 with the inter-sublattice tensor                      */
+  MMX_T_MEL = 512,       /* Eq.9 magnetoelastic field */
+  MMX_T_ALL = 1023
+};
+
+/* state fields for mmx_set_state / mmx_get_state */
+enum { MMX_F_M0 = 0, MMX_F_M1 = 1, MMX_F_U = 2, MMX_F_V = 3 };
+
+/* Runge-Kutta methods (Table 2; RK4 = classical, not in the table) */
+enum {
+  MMX_RK4 = 0,      /* classical 4th order, fixed step only            */
+  MMX_DP45 = 1,     /* Dormand-Prince 5(4), FSAL   (Table 2 row 5)     */
+  MMX_HEUN12 = 2,   /* Heun 2(1)                   (Table 2 row 1)     */
+  MMX_BS23 = 3,     /* Bogacki-Shampine 3(2), FSAL (Table 2 row 2)     */
+  MMX_CK45 = 4,     /* Cash-Karp 5(4)              (Table 2 row 3)     */
+  MMX_RKF45 = 5     /* Fehlberg 5(4)               (Table 2 row 4)     */
+};
+
+/* Per (sublattice, region) material parameters ("material parameters"). */
+typedef struct mmx_material {
+  double Ms;      /* saturation magnetisation, A/m; 0 = empty cell                     */
+  double A;       /* exchange stiffness A11, J/m                                       */
+  double alpha;   /* Gilbert damping                                                   */
+  double Ku1;     /* uniaxial anisotropy constant, J/m^3                               */
+  double Kc1;     /* cubic anisotropy constant, J/m^3                                  */
+  double D;       /* interfacial DMI strength of this sublattice, J/m^2                */
+  double B1, B2;  /* magnetoelastic coupling constants, J/m^3 (Eq.8-9)                 */
+  double pol;     /* spin polarisation of the current (Zhang-Li)                       */
+  double xi;      /* non-adiabaticity (Zhang-Li)                                       */
+  double gamma;   /* gyromagnetic ratio, rad/(T s); <= 0 selects 1.7595e11             */
+  double u[3];    /* uniaxial axis (unit vector)                                       */
+  double c1[3];   /* cubic axes c1, c2 (unit, orthogonal); c3 = c1 x c2                */
+  double c2[3];
+} mmx_material;
+
+/* Inter-sublattice coupling and grain-boundary scaling (Eq.3). */
+typedef struct mmx_coupling {
+  double A0;        /* homogeneous inter-sublattice exchange, J/m                      */
+  double A12;       /* inhomogeneous inter-sublattice exchange, J/m                    */
+  double latcon;    /* lattice constant a of Eq.3, m                                   */
+  double D_inter;   /* inter-sublattice interfacial DMI, J/m^2                         */
+  double scale_A11; /* factor on A11 between cells of different regions (1 = none)     */
+  double scale_A12; /* factor on A12 between cells of different regions                */
+} mmx_coupling;
+
+/* Elastic medium (Eq.7) and one optional time-harmonic traction. */
+typedef struct mmx_elastic {
+  double C11, C12, C44;   /* cubic stiffness constants, Pa                             */
+  double rho;             /* mass density, kg/m^3                                      */
+  int traction_face;      /* -1 none; 0:x- 1:x+ 2:y- 3:y+ 4:z- 5:z+                    */
+  double traction_vec[3]; /* direction of t in sigma.n = t                             */
+  double traction_amp;    /* Pa                                                        */
+  double traction_freq;   /* Hz; t(t) = amp * sin(2 pi freq t) * vec                   */
+} mmx_elastic;
+
+typedef struct mmx_rk_opts {
+  int method;          /* MMX_DP45, ... (embedded pairs); MMX_RK4 only with fixed_dt    */
+  int fixed_dt;        /* 1: every step accepted with dt = dt0 (parity / roofline runs) */
+  double dt0;          /* first (or fixed) step; <= 0: 0.01 / max|torque| (adaptive)    */
+  double tol;          /* accept iff err <= tol, err = dt*max_c |sum_j e_j k_j|_2       */
+  long long nsteps;    /* stop after this many accepted steps (<= 0: no limit)          */
+  double t_end;        /* stop when t >= t_end (<= 0: no limit)                         */
+  double torque_stop;  /* stop when max|tau| < torque_stop [1/s] (<= 0: off)            */
+  long long max_attempts; /* hard cap on attempted steps (<= 0: 1000000)                */
+} mmx_rk_opts;
+
+typedef struct mmx_rk_stats {
+  long long accepted, rejected;
+  double t;          /* simulation time after the call                                 */
+  double dt;         /* step size proposed for the next step                           */
+  double last_err;   /* error estimate of the last attempted step                      */
+  double max_torque; /* max_c |tau_c| [1/s] at the last accepted state (FSAL methods)  */
+  long long launches;/* CUDA kernels launched by this call                             */
+} mmx_rk_stats;
+
+/* ---- life cycle ------------------------------------------------------------------- */
+
+/* Message of the last failing call made by this thread ("" if none). */
+const char* mmx_last_error(void);
+
+/* Library version string. */
+const char* mmx_version(void);
+
+/* Create a world on the current CUDA device.
+ *   grid[3]     = (Nx, Ny, Nz) cells, each >= 1
+ *   cellsize[3] = (dx, dy, dz) in m
+ *   pbc[3]      = number of periodic image repetitions per axis used by the demag kernel;
+ *                 0 = open axis.  A periodic axis must have a power-of-two size.
+ *   n_sublattices = 1 (ferromagnet) or 2 (antiferro-/ferrimagnet)
+ *   cuda_stream = cudaStream_t (as void*) on which all work is enqueued, or NULL
+ * Materials default to Ms = 0 everywhere until mmx_set_material is called. */
+int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[3],
+                     int n_sublattices, void* cuda_stream, mmx_world** out);
+int mmx_world_destroy(mmx_world* w);
+
+/* ---- parameters --------------------------------------------------------------------- */
+
+/* Region index of every cell, [Nz][Ny][Nx] uint16 (P:L92 per-cell parameters, stored as a
+ * region map + table).  n_regions >= 1; region_of_cell == NULL resets to one region. */
+int mmx_set_regions(mmx_world* w, const uint16_t* region_of_cell, int mem, int n_regions);
+/* Material of (sublattice, region); call after mmx_set_regions. */
+int mmx_set_material(mmx_world* w, int sublattice, int region, const mmx_material* mat);
+int mmx_set_coupling(mmx_world* w, const mmx_coupling* c);
+int mmx_set_bext(mmx_world* w, const double B[3]);     /* uniform external field, T */
+int mmx_set_current(mmx_world* w, const double J[3]);  /* Zhang-Li current density, A/m^2 */
+/* Enable elastodynamics (adds the fields U, V to the integrated state); NULL disables. */
+int mmx_set_elastic(mmx_world* w, const mmx_elastic* e);
+/* Switch the magnetostatic term on/off for stepping (default on once the kernel exists). */
+int mmx_enable_demag(mmx_world* w, int on);
+
+/* Copy a state field in / out: `field` = MMX_F_*; buf is fp32 [3][Nz][Ny][Nx]. */
+int mmx_set_state(mmx_world* w, int field, const float* buf, int mem);
+int mmx_get_state(mmx_world* w, int field, float* buf, int mem);
+int mmx_set_time(mmx_world* w, double t);
+int mmx_get_time(mmx_world* w, double* t);
+
+/* ---- magnetostatic kernel ---------------------------------------------------------------- */
+
+/* Build the demagnetising tensor: Newell's analytic cell-cell tensor for
+ * offsets closer than analytic_cutoff_cells * max(cellsize) (<= 0 selects 32), an
+ * asymptotic (quadrature of the point-dipole tensor) form beyond; periodic images summed
+ * on periodic axes.  The tensor is transformed (fp64, host), scaled by -mu0 / P and stored
+ * as a real fp32 octant on the device.  One-time setup, not on the timed path. */
+int mmx_demag_kernel_init(mmx_world* w, double analytic_cutoff_cells);
+
+/* Host-only helper used by the tests: demag tensor N_ij (6 components xx,yy,zz,xy,xz,yz) on
+ * the non-negative octant of offsets, fp64 [6][n2][n1][n0], for an open (pbc=0) or periodic
+ * world.  n[a] = grid[a] on open axes, grid[a]/2+1 on periodic ones.  Needs no GPU. */
+int mmx_newell_tensor_host(const int grid[3], const double cellsize[3], const int pbc[3],
+                           double analytic_cutoff_cells, double* out, long long out_len);
+
+/* Host-only helper used by the tests: the real kernel spectrum as stored on the device,
+ * fp32 [6][KZ][KY][XP] with the factor -mu0/(Px Py Pz) folded in.  dims_out[5] receives
+ * (Px, Py, Pz, XP, total element count); call with out == NULL to query the sizes. */
+int mmx_kernel_spectrum_host(const int grid[3], const double cellsize[3], const int pbc[3],
+                             double analytic_cutoff_cells, float* out, long long out_len,
+                             long long dims_out[5]);
+
+/* ---- evaluation ------------------------------------------------------------------------ */
+
+/* Effective field of one sublattice, restricted to term_mask, of the current state (T). */
+int mmx_eval_heff(mmx_world* w, int sublattice, unsigned term_mask, float* out, int mem);
+/* Torque dm/dt (Eq.1-2 + Zhang-Li) of one sublattice for the current state (1/s), all
+ * enabled terms. */
+int mmx_eval_torque(mmx_world* w, int sublattice, float* out, int mem);
+/* Elastic right-hand side: acceleration (f_el + sum_s f_mel)/rho  (Eq.7-8), m/s^2. */
+int mmx_eval_accel(mmx_world* w, float* out, int mem);
+/* Energy (J) of the terms in term_mask summed over sublattices, fp64 accumulation. */
+int mmx_energy(mmx_world* w, unsigned term_mask, double* joule_out);
+/* (1/2 sum sigma:eps V, 1/2 sum rho v^2 V) */
+int mmx_elastic_energy(mmx_world* w, double* strain_energy, double* kinetic_energy);
+/* max over cells and sublattices of |tau| (1/s). */
+int mmx_max_torque(mmx_world* w, double* out);
+
+/* ---- time stepping --------------------------------------------------------------------- */
+
+/* nsteps classical RK4 steps of size dt (BASELINE config 1 protocol). */
+int mmx_step_rk4(mmx_world* w, double dt, long long nsteps);
+/* Embedded Runge-Kutta stepping (Table 2; default Dormand-Prince).  stats may be NULL
+ * (then the call is asynchronous when opts->fixed_dt && nsteps > 0). */
+int mmx_step_rk45(mmx_world* w, const mmx_rk_opts* opts, mmx_rk_stats* stats);
+/* Error estimates of the most recent attempted steps (newest last); returns the number
+ * written through *n_out (at most n). */
+int mmx_get_err_history(mmx_world* w, double* host_out, int n, int* n_out);
+
+/* Number of device bytes owned by the world. */
+int mmx_device_bytes(mmx_world* w, long long* bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MMX_H */

@@ -1,0 +1,401 @@
+// local.cu -- fused local effective field + torque + Runge-Kutta stage combination + error /
+// max-torque reduction, and the device-side step controller.
+//
+// Per cell c of sublattice s (partner sublattice s'):
+//   B_exch  = sum_n 2 A_cn /(Ms_c h_n^2) (m_n - m_c)                  Eq.3 term 1
+//   B_A12   = sum_n A12_cn /(Ms_c h_n^2) (m'_n - m'_c)                Eq.3 term 2
+//   B_A0    = 4 A0 /(a^2 Ms_c) m'_c                                    Eq.3 term 3
+//   B_DMI   = sum_{n in +-x,+-y} D_cn /(Ms_c h_n) (z x e_cn) x m_n     Eq.4, interfacial subset
+//   B_anis  = 2Ku1/Ms (u.m) u  - 2Kc1/Ms sum_i (c_i.m)[(c_j.m)^2+(c_k.m)^2] c_i
+//   B_mel   = -2/Ms [B1 eps_ii m_i + B2 (eps_ij m_j + eps_ik m_k)]     Eq.9
+//   B_eff   = sum of the above + B_ext + B_demag
+//   tau     = -gamma/(1+alpha^2) [m x B + alpha m x (m x B)]           Eq.2
+//           + Zhang-Li torque
+// A neighbour takes part only if it lies in the grid (after periodic wrap) and has Ms > 0
+// ("open" boundary = the pair is dropped).  A_cn, D_cn are harmonic means; A_cn, A12_cn carry
+// the region-pair scale factor across grain boundaries.
+// The epilogue forms the next stage state  normalise(y0 + sum_j (dt a_ij) k_j)  (Table 2,
+// P:L122-131) and, on the last stage, the embedded error  max_c |sum_j (dt e_j) k_j|_2.
+#include <cstdio>
+
+#include "mmx_internal.h"
+
+namespace {
+
+struct V3 {
+  float x, y, z;
+};
+__device__ __forceinline__ V3 v3(float x, float y, float z) { V3 r = {x, y, z}; return r; }
+__device__ __forceinline__ V3 operator+(V3 a, V3 b) { return v3(a.x + b.x, a.y + b.y, a.z + b.z); }
+__device__ __forceinline__ V3 operator-(V3 a, V3 b) { return v3(a.x - b.x, a.y - b.y, a.z - b.z); }
+__device__ __forceinline__ V3 operator*(float s, V3 a) { return v3(s * a.x, s * a.y, s * a.z); }
+__device__ __forceinline__ V3 fma3(float s, V3 a, V3 b) { return v3(fmaf(s, a.x, b.x), fmaf(s, a.y, b.y), fmaf(s, a.z, b.z)); }
+__device__ __forceinline__ float dot(V3 a, V3 b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }
+__device__ __forceinline__ V3 cross(V3 a, V3 b) {
+  return v3(fmaf(a.y, b.z, -a.z * b.y), fmaf(a.z, b.x, -a.x * b.z), fmaf(a.x, b.y, -a.y * b.x));
+}
+__device__ __forceinline__ V3 ld3(const float* p, size_t N, size_t i) { return v3(p[i], p[N + i], p[2 * N + i]); }
+__device__ __forceinline__ void st3(float* p, size_t N, size_t i, V3 v) { p[i] = v.x; p[N + i] = v.y; p[2 * N + i] = v.z; }
+__device__ __forceinline__ float harm(float a, float b) {
+  float s = a + b;
+  return s != 0.f ? 2.f * a * b / s : 0.f;
+}
+
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// block-wide max of a non-negative float, result atomically folded into *target (bit pattern).
+// NaN is mapped to +inf bits + 1 so that it survives the unsigned max and is seen by the controller.
+__device__ __forceinline__ void block_max_to(float v, unsigned* target) {
+  __shared__ unsigned smax[32];
+  unsigned bits = (v != v) ? 0x7fc00000u : __float_as_uint(v);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) bits = max(bits, __shfl_xor_sync(0xffffffffu, bits, o));
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) smax[wid] = bits;
+  __syncthreads();
+  if (wid == 0) {
+    const int nw = (blockDim.x + 31) >> 5;
+    bits = lane < nw ? smax[lane] : 0u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bits = max(bits, __shfl_xor_sync(0xffffffffu, bits, o));
+    if (lane == 0 && bits != 0u) atomicMax(target, bits);
+  }
+  __syncthreads();
+}
+
+// neighbour index of cell (ix,iy,iz) along axis by d = +-1, or -1 when outside an open axis
+__device__ __forceinline__ long long nbr(const LocalArgs& a, int ix, int iy, int iz, int axis, int d) {
+  int p[3] = {ix, iy, iz};
+  const int n[3] = {a.nx, a.ny, a.nz};
+  int q = p[axis] + d;
+  if (q < 0 || q >= n[axis]) {
+    if (!a.per[axis]) return -1;
+    q = (q + n[axis]) % n[axis];
+  }
+  p[axis] = q;
+  return ((long long)p[2] * a.ny + p[1]) * a.nx + p[0];
+}
+
+template <int S, bool REG>
+__global__ void __launch_bounds__(256) k_local(LocalArgs a) {
+  MmxCtrl* ctrl = a.ctrl;
+  if (!ctrl->active) return;
+  const int sel = ctrl->sel;
+  const size_t N = (size_t)a.nx * a.ny * a.nz;
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const float* yin = a.yin[sel];
+  float errv = 0.f, tqv = 0.f;
+  bool bad = false;
+  if (i < N) {
+    const int ix = (int)(i % a.nx), iy = (int)((i / a.nx) % a.ny), iz = (int)(i / ((size_t)a.nx * a.ny));
+    const int rc = REG ? a.reg[i] : 0;
+    long long ni[6];
+    int rn[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+      ni[q] = nbr(a, ix, iy, iz, q >> 1, (q & 1) ? -1 : +1);
+      rn[q] = (REG && ni[q] >= 0) ? a.reg[ni[q]] : rc;
+    }
+    V3 mc[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) mc[s] = ld3(yin + (size_t)s * 3 * N, N, i);
+
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      if (a.heff_out || a.tau_out) {
+        if (s != a.heff_s) continue;
+      }
+      const int o = S == 2 ? 1 - s : s;
+      const float* P = a.mat + ((size_t)s * a.nreg + rc) * MMX_MATW;
+      const float Ms = P[MP_MS], iMs = P[MP_INVMS];
+      const float* ms_ = yin + (size_t)s * 3 * N;
+      const float* mo_ = yin + (size_t)o * 3 * N;
+      V3 B = v3(0.f, 0.f, 0.f);
+      V3 dm = v3(0.f, 0.f, 0.f);  // (u.grad) m for Zhang-Li
+      V3 tau = v3(0.f, 0.f, 0.f);
+      if (Ms > 0.f) {
+        const float Ac = P[MP_A], Dc = P[MP_D];
+        const float zlb = P[MP_ZLB];
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+          const int axis = q >> 1;
+          const float d = (q & 1) ? -1.f : 1.f;
+          V3 mn = mc[s];  // missing neighbour: centre value (only used by Zhang-Li)
+          if (ni[q] >= 0) {
+            const float* Pn = REG ? a.mat + ((size_t)s * a.nreg + rn[q]) * MMX_MATW : P;
+            if (Pn[MP_MS] > 0.f) {
+              mn = ld3(ms_, N, (size_t)ni[q]);
+              const bool same = rn[q] == rc;
+              if (a.terms & MMX_T_EXCH) {
+                const float wex = 2.f * harm(Ac, Pn[MP_A]) * (same ? 1.f : a.scaleA11) * iMs * a.inv_h2[axis];
+                B = fma3(wex, mn - mc[s], B);
+              }
+              if (axis < 2 && (a.terms & MMX_T_DMI)) {
+                const float wd = harm(Dc, Pn[MP_D]) * iMs * a.inv_h[axis] * d;
+                // (z x (d e_axis)) x m_n = d (m_z e_axis - m_axis z)
+                if (axis == 0) { B.x = fmaf(wd, mn.z, B.x); B.z = fmaf(-wd, mn.x, B.z); }
+                else { B.y = fmaf(wd, mn.z, B.y); B.z = fmaf(-wd, mn.y, B.z); }
+              }
+              if (S == 2) {
+                if (a.terms & (MMX_T_A12 | MMX_T_DMI_INTER)) {
+                  const V3 on = ld3(mo_, N, (size_t)ni[q]);
+                  if (a.terms & MMX_T_A12) {
+                    const float w12 = a.A12 * (same ? 1.f : a.scaleA12) * iMs * a.inv_h2[axis];
+                    B = fma3(w12, on - mc[o], B);
+                  }
+                  if (axis < 2 && (a.terms & MMX_T_DMI_INTER)) {
+                    const float wd = a.Dinter * iMs * a.inv_h[axis] * d;
+                    if (axis == 0) { B.x = fmaf(wd, on.z, B.x); B.z = fmaf(-wd, on.x, B.z); }
+                    else { B.y = fmaf(wd, on.z, B.y); B.z = fmaf(-wd, on.y, B.z); }
+                  }
+                }
+              }
+            }
+          }
+          if (a.has_J) {
+            // central difference: (m_+ - m_-)/(2h) weighted by u_axis = zlb * J_axis
+            const float wu = zlb * a.J[axis] * 0.5f * a.inv_h[axis] * d;
+            dm = fma3(wu, mn, dm);
+          }
+        }
+        if (S == 2 && (a.terms & MMX_T_A0)) B = fma3(a.a0pref * iMs, mc[o], B);
+        if (a.terms & MMX_T_ANIS_U) {
+          const V3 u = v3(P[MP_UX], P[MP_UY], P[MP_UZ]);
+          B = fma3(P[MP_KU2] * dot(u, mc[s]), u, B);
+        }
+        if ((a.terms & MMX_T_ANIS_C) && P[MP_KC2] != 0.f) {
+          const V3 c1 = v3(P[MP_C1X], P[MP_C1Y], P[MP_C1Z]);
+          const V3 c2 = v3(P[MP_C2X], P[MP_C2Y], P[MP_C2Z]);
+          const V3 c3 = v3(P[MP_C3X], P[MP_C3Y], P[MP_C3Z]);
+          const float a1 = dot(c1, mc[s]), a2 = dot(c2, mc[s]), a3 = dot(c3, mc[s]);
+          const float k = -P[MP_KC2];
+          B = fma3(k * a1 * (a2 * a2 + a3 * a3), c1, B);
+          B = fma3(k * a2 * (a3 * a3 + a1 * a1), c2, B);
+          B = fma3(k * a3 * (a1 * a1 + a2 * a2), c3, B);
+        }
+        if (a.terms & MMX_T_ZEEMAN) B = B + v3(a.bext[0], a.bext[1], a.bext[2]);
+        if ((a.terms & MMX_T_DEMAG) && a.bdemag) B = B + ld3(a.bdemag, N, i);
+        if ((a.terms & MMX_T_MEL) && a.strain) {
+          const float exx = a.strain[i], eyy = a.strain[N + i], ezz = a.strain[2 * N + i];
+          const float exy = a.strain[3 * N + i], exz = a.strain[4 * N + i], eyz = a.strain[5 * N + i];
+          const float p1 = -P[MP_MEL1], p2 = -P[MP_MEL2];
+          const V3 m = mc[s];
+          B.x += p1 * exx * m.x + p2 * (exy * m.y + exz * m.z);
+          B.y += p1 * eyy * m.y + p2 * (exy * m.x + eyz * m.z);
+          B.z += p1 * ezz * m.z + p2 * (exz * m.x + eyz * m.y);
+        }
+        // Eq.2
+        const V3 m = mc[s];
+        const V3 mxB = cross(m, B);
+        const V3 mxmxB = cross(m, mxB);
+        const float alpha = P[MP_ALPHA];
+        tau = (-P[MP_LLG]) * fma3(alpha, mxmxB, mxB);
+        if (a.has_J) {
+          // tau_ZL = -(1+alpha^2)^-1 [ (1 + xi alpha) m x (m x dm) + (xi - alpha) m x dm ]
+          const float xi = P[MP_XI];
+          const V3 mxa = cross(m, dm);
+          const V3 mxmxa = cross(m, mxa);
+          const float inv = -1.f / (1.f + alpha * alpha);
+          tau = fma3(inv * (1.f + xi * alpha), mxmxa, tau);
+          tau = fma3(inv * (xi - alpha), mxa, tau);
+        }
+      }
+      if (a.heff_out) { st3(a.heff_out, N, i, B); continue; }
+      if (a.tau_out) { st3(a.tau_out, N, i, tau); continue; }
+      st3(a.kout[sel] + (size_t)s * 3 * N, N, i, tau);
+      if (a.do_tq) {
+        const float t2 = dot(tau, tau);
+        tqv = fmaxf(tqv, sqrtf(t2));
+        bad |= !(t2 == t2);
+      }
+      if (a.ynext[0]) {
+        const float* ca = ctrl->ca[a.combine_row];
+        V3 y = ld3(a.y0[sel] + (size_t)s * 3 * N, N, i);
+        V3 acc = v3(0.f, 0.f, 0.f);
+        for (int j = 0; j < a.n_prev; ++j) {
+          const float cj = ca[j];
+          if (cj != 0.f) acc = fma3(cj, ld3(a.kprev[sel][j] + (size_t)s * 3 * N, N, i), acc);
+        }
+        acc = fma3(ca[a.stage], tau, acc);
+        y = y + acc;
+        const float n2 = dot(y, y);
+        if (n2 > 0.f) y = (1.f / sqrtf(n2)) * y;
+        st3(a.ynext[sel] + (size_t)s * 3 * N, N, i, y);
+      }
+      if (a.do_err) {
+        const float* ce = ctrl->ce;
+        V3 e = v3(0.f, 0.f, 0.f);
+        for (int j = 0; j < a.n_prev; ++j) {
+          const float cj = ce[j];
+          if (cj != 0.f) e = fma3(cj, ld3(a.kprev[sel][j] + (size_t)s * 3 * N, N, i), e);
+        }
+        e = fma3(ce[a.stage], tau, e);
+        const float e2 = dot(e, e);
+        errv = fmaxf(errv, sqrtf(e2));
+        bad |= !(e2 == e2);
+      }
+    }
+  }
+  if (bad) errv = tqv = __int_as_float(0x7fc00000);
+  if (a.do_err) block_max_to(errv, &ctrl->err_bits);
+  if (a.do_tq) block_max_to(tqv, &ctrl->tq_bits);
+}
+
+// y_next = project(y0 + ca[row][0] * k1) for all vectors (m normalised, u and v not)
+__global__ void __launch_bounds__(256) k_combine1(const float* y0a, const float* y0b, const float* k1a,
+                                                  const float* k1b, float* yna, float* ynb, int row, int S,
+                                                  int nvec, size_t N, MmxCtrl* ctrl) {
+  if (!ctrl->active) return;
+  const int sel = ctrl->sel;
+  const float* y0 = sel ? y0b : y0a;
+  const float* k1 = sel ? k1b : k1a;
+  float* yn = sel ? ynb : yna;
+  const float c = ctrl->ca[row][0];
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  for (int v = 0; v < nvec; ++v) {
+    const size_t b = (size_t)v * 3 * N;
+    V3 y = fma3(c, ld3(k1 + b, N, i), ld3(y0 + b, N, i));
+    if (v < S) {
+      const float n2 = dot(y, y);
+      if (n2 > 0.f) y = (1.f / sqrtf(n2)) * y;
+    }
+    st3(yn + b, N, i, y);
+  }
+}
+
+// mode 0: begin of an attempt (fill the coefficient tables from dt, clear the reductions)
+// mode 1: end of an attempt (accept / reject, new dt, bookkeeping)
+// mode 2: re-arm (active = 1) after a stepping call
+// mode 3: first step size from max torque: dt = 0.01 / max|tau| (only when dt <= 0)
+__global__ void k_controller(MmxCtrl* c, MmxTableau tab, int mode) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  if (mode == 2) { c->active = 1; return; }
+  if (mode == 3) {
+    if (c->dt <= 0.0) {
+      const double tq = (double)__uint_as_float(c->tq_bits);
+      c->dt = tq > 0.0 ? 0.01 / tq : 1e-15;
+    }
+    c->max_torque = (double)__uint_as_float(c->tq_bits);
+    return;
+  }
+  if (!c->active) return;
+  if (mode == 0) {
+    double dt = c->dt;
+    if (c->t_end > 0.0 && c->t + dt > c->t_end) dt = c->t_end - c->t;
+    c->dt = dt;
+    for (int i = 0; i < MMX_MAX_STAGES; ++i) {
+      for (int j = 0; j < MMX_MAX_STAGES; ++j) c->ca[i][j] = (float)(dt * tab.a[i][j]);
+      c->ce[i] = (float)(dt * tab.e[i]);
+      c->cc[i] = (float)tab.c[i];
+    }
+    c->err_bits = 0u;
+    c->tq_bits = 0u;
+    return;
+  }
+  // mode 1
+  const unsigned eb = c->err_bits, tb = c->tq_bits;
+  const double err = (double)__uint_as_float(eb);
+  const bool bad = eb >= 0x7f800000u || tb >= 0x7f800000u;
+  c->err_last = err;
+  c->hist[c->hist_n % MMX_HIST] = err;
+  c->hist_n++;
+  c->attempts++;
+  bool accept = c->fixed || !tab.embedded || err <= c->tol;
+  if (bad) { c->nan_flag = 1; c->active = 0; accept = false; }
+  double dt_new = c->dt;
+  if (!c->fixed && tab.embedded) {
+    double fac = 2.0;
+    if (err > 0.0) {
+      fac = pow(c->tol / err, 1.0 / (double)c->order);
+      fac = fmin(2.0, fmax(0.5, fac));
+    }
+    dt_new = c->dt * 0.8 * fac;
+  }
+  if (accept) {
+    c->t += c->dt;
+    c->accepted++;
+    c->sel ^= 1;
+    c->max_torque = (double)__uint_as_float(tb);
+    if (c->target_accepted > 0 && c->accepted >= c->target_accepted) c->active = 0;
+    if (c->t_end > 0.0 && c->t >= c->t_end * (1.0 - 1e-14)) c->active = 0;
+    if (tab.fsal && c->torque_stop > 0.0 && c->max_torque < c->torque_stop) c->active = 0;
+  } else if (!bad) {
+    c->rejected++;
+  }
+  c->dt = dt_new;
+}
+
+// energies: E = -c_term V sum_c Ms_c m_c . B_term,c ; fp64 accumulation
+__global__ void __launch_bounds__(256) k_dot_energy(const float* m, const float* B, const uint16_t* reg,
+                                                    const float* mat, int nreg, size_t N, double* acc) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double v = 0.0;
+  if (i < N) {
+    const int r = reg ? reg[i] : 0;
+    const double Ms = mat[(size_t)r * MMX_MATW + MP_MS];
+    v = Ms * ((double)m[i] * B[i] + (double)m[N + i] * B[N + i] + (double)m[2 * N + i] * B[2 * N + i]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __shared__ double sm[8];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) sm[wid] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int k = 0; k < 8; ++k) t += sm[k];
+    atomicAdd(acc, t);
+  }
+}
+
+}  // namespace
+
+int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
+  const size_t N = w->N;
+  const unsigned blocks = (unsigned)((N + 255) / 256);
+  const bool reg = w->nreg > 1;
+  if (w->S == 1) {
+    if (reg) k_local<1, true><<<blocks, 256, 0, w->stream>>>(a);
+    else k_local<1, false><<<blocks, 256, 0, w->stream>>>(a);
+  } else {
+    if (reg) k_local<2, true><<<blocks, 256, 0, w->stream>>>(a);
+    else k_local<2, false><<<blocks, 256, 0, w->stream>>>(a);
+  }
+  w->launches++;
+  MMX_CUDA(cudaGetLastError());
+  return MMX_OK;
+}
+
+int mmx_combine_launch(mmx_world* w, const float* const y0[2], const float* const k1[2],
+                       float* const ynext[2], int row) {
+  const unsigned blocks = (unsigned)((w->N + 255) / 256);
+  k_combine1<<<blocks, 256, 0, w->stream>>>(y0[0], y0[1], k1[0], k1[1], ynext[0], ynext[1], row, w->S,
+                                            w->nvec, w->N, w->d_ctrl);
+  w->launches++;
+  MMX_CUDA(cudaGetLastError());
+  return MMX_OK;
+}
+
+int mmx_controller_launch(mmx_world* w, const MmxTableau& tab, int mode) {
+  k_controller<<<1, 32, 0, w->stream>>>(w->d_ctrl, tab, mode);
+  w->launches++;
+  MMX_CUDA(cudaGetLastError());
+  return MMX_OK;
+}
+
+// sum over sublattices of  Ms m . B  for the field already stored in w->scratch (per sublattice
+// call): helper used by mmx_energy in api.cu
+int mmx_energy_launch(mmx_world* w, unsigned s, const float* B, double* dev_acc) {
+  const unsigned blocks = (unsigned)((w->N + 255) / 256);
+  k_dot_energy<<<blocks, 256, 0, w->stream>>>(w->Y[w->sel_host] + (size_t)s * 3 * w->N, B,
+                                              w->nreg > 1 ? w->d_reg : nullptr,
+                                              w->d_mat + (size_t)s * w->nreg * MMX_MATW, w->nreg, w->N, dev_acc);
+  w->launches++;
+  MMX_CUDA(cudaGetLastError());
+  return MMX_OK;
+}
