@@ -221,6 +221,14 @@ int mmx_step_rk45(mmx_world* w, const mmx_rk_opts* opts, mmx_rk_stats* stats);
  * written through *n_out (at most n). */
 int mmx_get_err_history(mmx_world* w, double* host_out, int n, int* n_out);
 
+/* Built-in kernel timer: while enabled, every kernel launch is bracketed by CUDA events on the
+ * world's stream.  mmx_profile_read synchronises, sums the elapsed milliseconds and launch counts
+ * per kernel category into ms_out[n] / count_out[n] (n >= 11) and clears the records.
+ * Categories: 0 demag x_fwd, 1 mid_fwd, 2 inner (fwd * K * inv), 3 mid_inv, 4 x_inv,
+ * 5 local field/torque/RK, 6 RK combine, 7 controller, 8 strain, 9 elastic RHS, 10 energy. */
+int mmx_profile_enable(mmx_world* w, int on);
+int mmx_profile_read(mmx_world* w, double* ms_out, long long* count_out, int n);
+
 /* Number of device bytes owned by the world. */
 int mmx_device_bytes(mmx_world* w, long long* bytes);
 

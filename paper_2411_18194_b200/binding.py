@@ -23,6 +23,10 @@ RK4, DP45, HEUN12, BS23, CK45, RKF45 = 0, 1, 2, 3, 4, 5
 FACES = {"x-": 0, "x+": 1, "y-": 2, "y+": 3, "z-": 4, "z+": 5}
 
 
+PROFILE_CATEGORIES = ("demag_x_fwd", "demag_mid_fwd", "demag_inner", "demag_mid_inv", "demag_x_inv",
+                      "local", "combine", "controller", "strain", "elastic", "energy")
+
+
 class MmxError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__("mmx status %d: %s" % (code, msg))
@@ -90,6 +94,8 @@ PROTOTYPES = {
     "mmx_step_rk4": (C.c_int, [_W, C.c_double, C.c_longlong]),
     "mmx_step_rk45": (C.c_int, [_W, C.POINTER(RkOpts), C.POINTER(RkStats)]),
     "mmx_get_err_history": (C.c_int, [_W, _D3, C.c_int, _I3]),
+    "mmx_profile_enable": (C.c_int, [_W, C.c_int]),
+    "mmx_profile_read": (C.c_int, [_W, _D3, C.POINTER(C.c_longlong), C.c_int]),
     "mmx_device_bytes": (C.c_int, [_W, C.POINTER(C.c_longlong)]),
 }
 
@@ -308,6 +314,17 @@ class World:
         got = C.c_int()
         _check(self.lib.mmx_get_err_history(self.h, buf, n, C.byref(got)))
         return np.array(buf[:got.value])
+
+    def profile_enable(self, on=True):
+        _check(self.lib.mmx_profile_enable(self.h, 1 if on else 0))
+
+    def profile_read(self):
+        """dict category -> (total ms, launches) since profile_enable / the last read."""
+        n = len(PROFILE_CATEGORIES)
+        ms = (C.c_double * n)()
+        cnt = (C.c_longlong * n)()
+        _check(self.lib.mmx_profile_read(self.h, ms, cnt, n))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(PROFILE_CATEGORIES)}
 
     def device_bytes(self):
         b = C.c_longlong()

@@ -520,6 +520,7 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
   w->d_ctrl = nullptr; w->d_acc = nullptr;
   w->sel_host = 0; w->k1_valid = false; w->k1_method = -1;
   w->dev_bytes = 0; w->launches = 0;
+  w->prof = false;
   int rc = dev_alloc(w, &w->d_mat, (size_t)w->S * MMX_MATW);
   if (!rc) rc = dev_alloc(w, &w->d_ctrl, 1);
   if (!rc) rc = dev_alloc(w, &w->d_acc, 64);
@@ -898,6 +899,31 @@ int mmx_get_err_history(mmx_world* w, double* host_out, int n, int* n_out) {
   MMX_CUDA(cudaStreamSynchronize(w->stream));
   for (int q = 0; q < have; ++q) host_out[q] = hist[(size_t)(h.hist_n - have + q) % MMX_HIST];
   *n_out = have;
+  return MMX_OK;
+}
+
+int mmx_profile_enable(mmx_world* w, int on) {
+  if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
+  cudaStreamSynchronize(w->stream);
+  for (auto& r : w->prof_recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+  w->prof_recs.clear();
+  w->prof = on != 0;
+  return MMX_OK;
+}
+
+int mmx_profile_read(mmx_world* w, double* ms_out, long long* count_out, int n) {
+  if (!w || !ms_out || !count_out || n < PK_COUNT) return mmx_fail(MMX_EINVAL, "need room for %d categories", PK_COUNT);
+  MMX_CUDA(cudaStreamSynchronize(w->stream));
+  for (int i = 0; i < n; ++i) { ms_out[i] = 0.0; count_out[i] = 0; }
+  for (auto& r : w->prof_recs) {
+    float ms = 0.f;
+    MMX_CUDA(cudaEventElapsedTime(&ms, r.e0, r.e1));
+    ms_out[r.cat] += ms;
+    count_out[r.cat] += 1;
+    cudaEventDestroy(r.e0);
+    cudaEventDestroy(r.e1);
+  }
+  w->prof_recs.clear();
   return MMX_OK;
 }
 

@@ -310,6 +310,7 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     constexpr int L = lines_for(PP);                                                      \
     size_t sm = sizeof(float2) * PP * (L | 1);                                            \
     if (int rc = set_smem(k_x_fwd<PP>, sm)) return rc;                                    \
+    ProfScope ps(w, PK_X_FWD);                                                             \
     k_x_fwd<PP><<<(rows + 2 * L - 1) / (2 * L), block_for(PP), sm, st>>>(xa);             \
   }
   MMX_SWITCH_P(d.px, 2, CALL_XF)
@@ -326,6 +327,7 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     size_t sm = sizeof(float2) * PP * L;                                                  \
     if (int rc = set_smem(k_mid<PP, -1>, sm)) return rc;                                  \
     dim3 g((d.xc + L - 1) / L, 3 * d.nz);                                                 \
+    ProfScope ps(w, PK_MID_FWD);                                                           \
     k_mid<PP, -1><<<g, block_for(PP), sm, st>>>(ma);                                      \
   }
     MMX_SWITCH_P(d.py, 2, CALL_MF)
@@ -360,6 +362,7 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     size_t sm = sizeof(float2) * 3 * PP * L;                                              \
     if (int rc = set_smem(k_inner<PP>, sm)) return rc;                                    \
     dim3 g((d.xc + L - 1) / L, nouter);                                                   \
+    ProfScope ps(w, PK_INNER);                                                             \
     k_inner<PP><<<g, block_for(PP), sm, st>>>(ia);                                        \
   }
     MMX_SWITCH_P(Pin, 1, CALL_IN)
@@ -377,6 +380,7 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     size_t sm = sizeof(float2) * PP * L;                                                  \
     if (int rc = set_smem(k_mid<PP, +1>, sm)) return rc;                                  \
     dim3 g((d.xc + L - 1) / L, 3 * d.nz);                                                 \
+    ProfScope ps(w, PK_MID_INV);                                                           \
     k_mid<PP, +1><<<g, block_for(PP), sm, st>>>(ma);                                      \
   }
     MMX_SWITCH_P(d.py, 2, CALL_MI)
@@ -388,6 +392,7 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     constexpr int L = lines_for(PP);                                                      \
     size_t sm = sizeof(float2) * PP * (L | 1);                                            \
     if (int rc = set_smem(k_x_inv<PP>, sm)) return rc;                                    \
+    ProfScope ps(w, PK_X_INV);                                                             \
     k_x_inv<PP><<<(rows + 2 * L - 1) / (2 * L), block_for(PP), sm, st>>>(xa);             \
   }
   MMX_SWITCH_P(d.px, 2, CALL_XI)

@@ -222,6 +222,7 @@ __global__ void __launch_bounds__(256) k_elastic_energy(const float* eps, const 
 
 int mmx_strain_launch(mmx_world* w, const ElasticArgs& a) {
   const unsigned blocks = (unsigned)((w->N + 255) / 256);
+  ProfScope ps(w, PK_STRAIN);
   k_strain<<<blocks, 256, 0, w->stream>>>(a);
   w->launches++;
   MMX_CUDA(cudaGetLastError());
@@ -230,6 +231,7 @@ int mmx_strain_launch(mmx_world* w, const ElasticArgs& a) {
 
 int mmx_elastic_launch(mmx_world* w, const ElasticArgs& a) {
   const unsigned blocks = (unsigned)((w->N + 255) / 256);
+  ProfScope ps(w, PK_ELASTIC);
   k_elastic<<<blocks, 256, 0, w->stream>>>(a);
   w->launches++;
   MMX_CUDA(cudaGetLastError());

@@ -359,6 +359,7 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   const size_t N = w->N;
   const unsigned blocks = (unsigned)((N + 255) / 256);
   const bool reg = w->nreg > 1;
+  ProfScope ps(w, PK_LOCAL);
   if (w->S == 1) {
     if (reg) k_local<1, true><<<blocks, 256, 0, w->stream>>>(a);
     else k_local<1, false><<<blocks, 256, 0, w->stream>>>(a);
@@ -374,6 +375,7 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
 int mmx_combine_launch(mmx_world* w, const float* const y0[2], const float* const k1[2],
                        float* const ynext[2], int row) {
   const unsigned blocks = (unsigned)((w->N + 255) / 256);
+  ProfScope ps(w, PK_COMBINE);
   k_combine1<<<blocks, 256, 0, w->stream>>>(y0[0], y0[1], k1[0], k1[1], ynext[0], ynext[1], row, w->S,
                                             w->nvec, w->N, w->d_ctrl);
   w->launches++;
@@ -382,6 +384,7 @@ int mmx_combine_launch(mmx_world* w, const float* const y0[2], const float* cons
 }
 
 int mmx_controller_launch(mmx_world* w, const MmxTableau& tab, int mode) {
+  ProfScope ps(w, PK_CTRL);
   k_controller<<<1, 32, 0, w->stream>>>(w->d_ctrl, tab, mode);
   w->launches++;
   MMX_CUDA(cudaGetLastError());
@@ -392,6 +395,7 @@ int mmx_controller_launch(mmx_world* w, const MmxTableau& tab, int mode) {
 // call): helper used by mmx_energy in api.cu
 int mmx_energy_launch(mmx_world* w, unsigned s, const float* B, double* dev_acc) {
   const unsigned blocks = (unsigned)((w->N + 255) / 256);
+  ProfScope ps(w, PK_ENERGY);
   k_dot_energy<<<blocks, 256, 0, w->stream>>>(w->Y[w->sel_host] + (size_t)s * 3 * w->N, B,
                                               w->nreg > 1 ? w->d_reg : nullptr,
                                               w->d_mat + (size_t)s * w->nreg * MMX_MATW, w->nreg, w->N, dev_acc);

@@ -123,6 +123,15 @@ struct DemagPlan {
   bool ready;
 };
 
+// kernel categories of the built-in profiler (mmx_profile_*)
+enum { PK_X_FWD = 0, PK_MID_FWD, PK_INNER, PK_MID_INV, PK_X_INV, PK_LOCAL, PK_COMBINE, PK_CTRL, PK_STRAIN,
+       PK_ELASTIC, PK_ENERGY, PK_COUNT };
+
+struct ProfRec {
+  int cat;
+  cudaEvent_t e0, e1;
+};
+
 struct mmx_world {
   int grid[3];
   double cell[3];
@@ -156,6 +165,29 @@ struct mmx_world {
   int k1_method;
   long long dev_bytes;
   long long launches;
+  bool prof;
+  std::vector<ProfRec> prof_recs;
+};
+
+// RAII: brackets one kernel launch with CUDA events on the world's stream when profiling is on
+struct ProfScope {
+  mmx_world* w;
+  ProfRec r;
+  bool on;
+  ProfScope(mmx_world* w_, int cat) : w(w_), on(w_->prof) {
+    if (on) {
+      r.cat = cat;
+      cudaEventCreate(&r.e0);
+      cudaEventCreate(&r.e1);
+      cudaEventRecord(r.e0, w->stream);
+    }
+  }
+  ~ProfScope() {
+    if (on) {
+      cudaEventRecord(r.e1, w->stream);
+      w->prof_recs.push_back(r);
+    }
+  }
 };
 
 // error plumbing (api.cu)

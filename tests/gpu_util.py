@@ -1,0 +1,39 @@
+"""Helpers of the GPU parity tests: build the CUDA world and the oracle world from the same
+seeded WorldSpec, and the error measures of BASELINE.json's north_star (readings S27)."""
+import numpy as np
+
+import paper_2411_18194_b200 as mmx
+from oracle.world import World as OracleWorld
+
+FIELD_TOL = 1e-5   # per-cell relative field error (north_star)
+TRAJ_TOL = 1e-4    # max |delta m| after a fixed-step trajectory (north_star)
+
+
+def field_err(got, ref):
+    """max_c |dB_c|_2 / max(|B_c|_2, 0.1 RMS|B|)   (reading S27)."""
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    d = np.sqrt(((got - ref) ** 2).sum(axis=0))
+    n = np.sqrt((ref ** 2).sum(axis=0))
+    rms = np.sqrt((n ** 2).mean())
+    if rms == 0.0:
+        return float(d.max())
+    return float((d / np.maximum(n, 0.1 * rms)).max())
+
+
+def max_dm(a, b):
+    return float(np.abs(np.asarray(a, np.float64) - np.asarray(b, np.float64)).max())
+
+
+def pair(spec, demag_mode="fft", demag=None):
+    """(cuda world, oracle world) for one spec."""
+    if demag is not None:
+        spec = spec.copy()
+        spec.demag = demag
+    g = mmx.World.from_spec(spec)
+    o = OracleWorld(spec, demag_mode=demag_mode)
+    return g, o
+
+
+def gpu_m(g, S):
+    return [g.get_state(mmx.F_M0 + s) for s in range(S)]

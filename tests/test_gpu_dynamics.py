@@ -1,0 +1,135 @@
+"""GPU parity, dynamics: fixed-step trajectories of every config (reduced sizes here, the
+BASELINE.json sizes in test_gpu_fullsize.py) against the fp64 oracle: max |delta m| <= 1e-4
+(north_star), DP45 error estimates, the adaptive controller, |m| = 1."""
+import numpy as np
+import pytest
+
+import paper_2411_18194_b200 as mmx
+import workloads as wl
+from gpu_util import TRAJ_TOL, gpu_m, max_dm, pair
+
+pytestmark = pytest.mark.gpu
+
+
+def _compare_state(g, o, spec, tol=TRAJ_TOL):
+    for s in range(spec.S):
+        m = g.get_state(mmx.F_M0 + s)
+        assert max_dm(m, o.m[s]) <= tol, (s, max_dm(m, o.m[s]))
+        np.testing.assert_allclose((m.astype(np.float64) ** 2).sum(axis=0), 1.0, atol=1e-6)
+
+
+def test_c1_rk4_full_protocol():
+    """BASELINE config 1 exactly: 64x16x1, RK4, dt = 1e-13, 2000 steps."""
+    spec = wl.c1()
+    g, o = pair(spec)
+    g.step_rk4(1e-13, 2000)
+    o.step_rk4(1e-13, 2000)
+    _compare_state(g, o, spec)
+    assert abs(g.get_time() - 2000e-13) < 1e-20
+    g.destroy()
+
+
+@pytest.mark.parametrize("name,grid,nsteps", [("c2", (64, 64, 1), 200), ("c3", (128, 32, 1), 200),
+                                              ("c4", (32, 32, 8), 100), ("c4", (20, 12, 3), 50),
+                                              ("c5", (64, 32, 1), 200)])
+def test_dp45_fixed_step_trajectory(name, grid, nsteps):
+    spec = wl.make(name, grid)
+    dt = spec.integrator["dt"]
+    g, o = pair(spec)
+    st = g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=nsteps)
+    errs = o.step_dp45_fixed(dt, nsteps)
+    assert st["accepted"] == nsteps and st["rejected"] == 0
+    _compare_state(g, o, spec)
+    hist = g.get_err_history(nsteps)
+    assert len(hist) == nsteps
+    np.testing.assert_allclose(hist, errs, rtol=2e-2, atol=1e-9)
+    if spec.elastic is not None:
+        u, v = g.get_state(mmx.F_U), g.get_state(mmx.F_V)
+        assert np.abs(u - o.u).max() <= 1e-4 * max(np.abs(o.u).max(), 1e-30)
+        assert np.abs(v - o.v).max() <= 1e-4 * max(np.abs(o.v).max(), 1e-30)
+    g.destroy()
+
+
+def test_rk4_two_sublattice_with_current():
+    spec = wl.make("c3", (128, 32, 1))
+    g, o = pair(spec)
+    g.step_rk4(5e-15, 200)
+    o.step_rk4(5e-15, 200)
+    _compare_state(g, o, spec)
+    g.destroy()
+
+
+def test_split_calls_equal_one_call():
+    """FSAL bookkeeping across calls: 2 x 25 steps == 50 steps, bit for bit."""
+    spec = wl.make("c4", (16, 16, 4))
+    a = mmx.World.from_spec(spec)
+    b = mmx.World.from_spec(spec)
+    a.step_rk45(fixed_dt=True, dt0=1e-13, nsteps=50)
+    b.step_rk45(fixed_dt=True, dt0=1e-13, nsteps=25)
+    b.step_rk45(fixed_dt=True, dt0=1e-13, nsteps=25)
+    assert np.array_equal(a.get_state(mmx.F_M0), b.get_state(mmx.F_M0))
+    a.destroy(); b.destroy()
+
+
+def test_adaptive_controller_matches_oracle():
+    """Adaptive DP45 (controller reading S21): same accept/reject sequence and step sizes."""
+    spec = wl.make("c2", (32, 32, 1))
+    g, o = pair(spec)
+    n = 40
+    st = g.step_rk45(method=mmx.DP45, tol=1e-5, nsteps=n)
+    ref = o.run_dp45(tol=1e-5, nsteps=n)
+    assert st["accepted"] == n == ref["accepted"]
+    assert abs(st["rejected"] - ref["rejected"]) <= 1
+    assert abs(st["t"] - ref["t"]) <= 2e-3 * ref["t"]
+    _compare_state(g, o, spec, tol=5e-4)
+    g.destroy()
+
+
+def test_adaptive_t_end_and_reject_path():
+    spec = wl.make("c1", (32, 16, 1))
+    g, o = pair(spec)
+    # a far too large first step must be rejected and leave the state untouched
+    m0 = g.get_state(mmx.F_M0)
+    st = g.step_rk45(method=mmx.DP45, tol=1e-7, dt0=5e-11, max_attempts=1)
+    assert st["accepted"] == 0 and st["rejected"] == 1
+    assert np.array_equal(g.get_state(mmx.F_M0), m0)
+    st = g.step_rk45(method=mmx.DP45, tol=1e-5, t_end=2e-12)
+    assert abs(st["t"] - 2e-12) < 1e-20
+    o.run_dp45(tol=1e-5, t_end=2e-12)
+    g.destroy()
+
+
+def test_c1_relaxation_reaches_torque_threshold():
+    """BASELINE config 1: RK45 relaxation until max torque < 1e-4 (T, i.e. |tau|/gamma; S26)."""
+    spec = wl.c1()
+    g = mmx.World.from_spec(spec)
+    gamma = 1.7595e11
+    e0 = g.energy()
+    st = g.step_rk45(method=mmx.DP45, tol=1e-5, torque_stop=1e-4 * gamma, max_attempts=200000)
+    assert st["max_torque"] < 1e-4 * gamma
+    assert g.max_torque() < 1.5e-4 * gamma
+    assert g.energy() < e0
+    g.destroy()
+
+
+@pytest.mark.parametrize("method,order", [(mmx.RK4, 4), (mmx.DP45, 5), (mmx.HEUN12, 2), (mmx.BS23, 3),
+                                          (mmx.CK45, 5), (mmx.RKF45, 5)])
+def test_macrospin_closed_form_every_tableau(method, order):
+    """Table 2 methods on the damped macrospin: m_z(t) = tanh(alpha gamma B t/(1+alpha^2) + atanh m_z0)."""
+    spec = wl.make("c1", (4, 2, 1))
+    spec.demag = False
+    spec.mat["A"][:] = 0.0
+    spec.mat["alpha"][:] = 0.1
+    spec.bext = (0.0, 0.0, 1.0)
+    m = np.zeros_like(spec.m[0])
+    m[0], m[2] = np.sqrt(1 - 0.25), 0.5
+    spec.m = [m]
+    g = mmx.World.from_spec(spec)
+    gamma, alpha, B = 1.7595e11, 0.1, 1.0
+    T = 2e-11
+    n = {2: 4000, 3: 800, 4: 200, 5: 100}[order]
+    g.step_rk45(method=method, fixed_dt=True, dt0=T / n, nsteps=n)
+    mz = g.get_state(mmx.F_M0)[2]
+    ref = np.tanh(alpha * gamma * B * T / (1 + alpha ** 2) + np.arctanh(0.5))
+    assert np.abs(mz - ref).max() < 2e-5
+    g.destroy()

@@ -1,0 +1,171 @@
+"""GPU parity, fields: every effective-field term, the torque and the energies of the CUDA path
+(through the C-ABI) against the fp64 oracle on the same seeded inputs.  Sizes span several tiles
+and ragged tails; the bar is the north_star's per-cell relative field error 1e-5 (reading S27)."""
+import numpy as np
+import pytest
+
+import paper_2411_18194_b200 as mmx
+import workloads as wl
+from oracle import constants as oc
+from gpu_util import FIELD_TOL, field_err, pair
+
+pytestmark = pytest.mark.gpu
+
+TERMS = {"exch": mmx.T_EXCH, "dmi": mmx.T_DMI, "anis_u": mmx.T_ANIS_U, "anis_c": mmx.T_ANIS_C,
+         "zeeman": mmx.T_ZEEMAN, "demag": mmx.T_DEMAG, "a12": mmx.T_A12, "a0": mmx.T_A0,
+         "dmi_inter": mmx.T_DMI_INTER, "mel": mmx.T_MEL}
+
+
+def _rich_spec(name, grid, seed=7):
+    """A config with every parameter switched on and a random state, so each term is non-trivial."""
+    spec = wl.make(name, grid)
+    rng = np.random.default_rng(seed)
+    R = spec.n_regions
+    for s in range(spec.S):
+        spec.m[s] = wl.random_unit(rng, grid)
+        spec.mat["Ku1"][s] = 5e4 * (1 + s)
+        spec.mat["Kc1"][s] = 2e4
+        spec.mat["D"][s] = 1e-3 * (1 + 0.5 * s)
+        spec.mat["B1"][s] = -1e7
+        spec.mat["B2"][s] = -0.7e7
+        spec.mat["A"][s] = 1e-11 * (1 + 0.3 * rng.random(R))
+    spec.bext = (0.01, -0.02, 0.1)
+    if spec.S == 2:
+        spec.coupling.update(A0=-4e-13, A12=-1e-12, D_inter=0.5e-3, scale_A11=0.25, scale_A12=0.5)
+    return spec
+
+
+CASES = [("c1", (64, 16, 1)), ("c1", (20, 12, 1)), ("c2", (32, 32, 1)), ("c3", (48, 24, 1)),
+         ("c4", (16, 16, 8)), ("c4", (20, 12, 3)), ("c5", (40, 24, 1))]
+
+
+@pytest.mark.parametrize("name,grid", CASES)
+def test_each_field_term(name, grid):
+    spec = _rich_spec(name, grid)
+    if spec.elastic is not None:
+        rng = np.random.default_rng(3)
+        spec.u = (1e-12 * rng.standard_normal(spec.u.shape)).astype(np.float32)
+    g, o = pair(spec)
+    for s in range(spec.S):
+        ref = o.field_terms(s)
+        for tname, bit in TERMS.items():
+            if bit not in ref:
+                continue
+            got = g.eval_heff(s, bit)
+            e = field_err(got, ref[bit])
+            assert e < FIELD_TOL, (name, grid, s, tname, e)
+        tot = g.eval_heff(s, mmx.T_ALL)
+        e = field_err(tot, o.heff(s))
+        assert e < FIELD_TOL, (name, grid, s, "total", e)
+    g.destroy()
+
+
+@pytest.mark.parametrize("name,grid", CASES)
+def test_torque(name, grid):
+    spec = _rich_spec(name, grid)
+    if name in ("c1", "c4"):
+        spec.J = (2e11, -1e11, 0.0 if grid[2] == 1 else 3e11)
+        spec.mat["pol"][:] = 0.6
+        spec.mat["xi"][:] = 0.05
+    g, o = pair(spec)
+    for s in range(spec.S):
+        e = field_err(g.eval_torque(s), o.torque(s))
+        assert e < FIELD_TOL, (name, grid, s, e)
+    tq = g.max_torque()
+    ref = o.max_torque()
+    assert abs(tq - ref) <= 1e-5 * ref
+    g.destroy()
+
+
+def test_demag_against_direct_sum_definition():
+    """FFT demag of the CUDA path against the oracle's O(N^2) direct sum (the definition)."""
+    for grid, pbc in [((8, 8, 4), (0, 0, 0)), ((12, 5, 2), (0, 0, 0)), ((8, 8, 1), (2, 2, 0)), ((16, 4, 1), (1, 0, 0))]:
+        spec = wl.make("c4", grid)
+        spec.pbc = pbc
+        g, o = pair(spec, demag_mode="direct")
+        e = field_err(g.eval_heff(0, mmx.T_DEMAG), o.field_terms(0, terms=oc.T_DEMAG)[oc.T_DEMAG])
+        assert e < FIELD_TOL, (grid, pbc, e)
+        g.destroy()
+
+
+def test_demag_uniform_cube_is_one_third():
+    """Closed form: a uniformly magnetised cube has N = 1/3 on average (pins sign and scale end to end)."""
+    spec = wl.make("c4", (8, 8, 8))
+    spec.m[0][:] = 0
+    spec.m[0][2] = 1.0
+    g = mmx.World.from_spec(spec)
+    B = g.eval_heff(0, mmx.T_DEMAG)
+    Ms = spec.mat["Ms"][0, 0]
+    assert abs(B[2].mean() / (-oc.MU0 * Ms) - 1.0 / 3.0) < 1e-5
+    assert abs(B[0].mean()) < 1e-6 and abs(B[1].mean()) < 1e-6
+    g.destroy()
+
+
+def test_two_sublattice_demag_uses_vector_sum():
+    spec = _rich_spec("c3", (32, 16, 1))
+    spec.mat["Ms"][1] = 2.5e5   # ferrimagnet: different Ms per sublattice (S15)
+    g, o = pair(spec)
+    ref = o.field_terms(0, terms=oc.T_DEMAG)[oc.T_DEMAG]
+    for s in range(2):
+        assert field_err(g.eval_heff(s, mmx.T_DEMAG), ref) < FIELD_TOL
+    g.destroy()
+
+
+def test_empty_cells_and_regions():
+    """Ms = 0 holes: no field, no torque there; neighbours drop the pair (open boundary, S9)."""
+    spec = _rich_spec("c3", (40, 20, 1))
+    R = spec.n_regions
+    hole = np.arange(R) % 3 == 0
+    for s in range(2):
+        spec.mat["Ms"][s, hole] = 0.0
+    g, o = pair(spec)
+    for s in range(2):
+        got, ref = g.eval_heff(s, mmx.T_ALL & ~mmx.T_DEMAG), o.heff(s, terms=oc.T_ALL & ~oc.T_DEMAG)
+        assert field_err(got, ref) < FIELD_TOL
+        mask = hole[spec.regions]
+        assert np.all(got[:, mask] == 0.0)
+        tq = g.eval_torque(s)
+        assert np.all(tq[:, mask] == 0.0)
+        assert field_err(tq, o.torque(s)) < FIELD_TOL
+    g.destroy()
+
+
+@pytest.mark.parametrize("name,grid", [("c2", (32, 32, 1)), ("c3", (48, 24, 1)), ("c4", (16, 16, 8)), ("c5", (40, 24, 1))])
+def test_energy(name, grid):
+    spec = _rich_spec(name, grid)
+    g, o = pair(spec)
+    for tname, bit in TERMS.items():
+        ref = o.energy(bit)
+        got = g.energy(bit)
+        scale = max(abs(o.energy(oc.T_EXCH)), abs(ref), 1e-30)
+        assert abs(got - ref) <= 2e-6 * scale, (tname, got, ref)
+    assert abs(g.energy() - o.energy()) <= 2e-6 * abs(o.energy(oc.T_EXCH))
+    g.destroy()
+
+
+def test_elastic_acceleration_and_energy():
+    spec = _rich_spec("c5", (40, 24, 1))
+    rng = np.random.default_rng(11)
+    spec.u = (1e-12 * rng.standard_normal(spec.u.shape)).astype(np.float32)
+    spec.v = (1e-1 * rng.standard_normal(spec.v.shape)).astype(np.float32)
+    g, o = pair(spec)
+    t = 3.0e-11
+    g.set_time(t)
+    ref = o.acceleration(o.m, o.u, t)
+    assert field_err(g.eval_accel(), ref) < FIELD_TOL
+    es, ek = g.elastic_energy()
+    res, rek = o.elastic_energy()
+    assert abs(es - res) <= 1e-5 * abs(res) and abs(ek - rek) <= 1e-5 * abs(rek)
+    g.destroy()
+
+
+def test_elastic_3d_and_periodic():
+    spec = _rich_spec("c5", (12, 10, 6))
+    spec.pbc = (0, 1, 0)
+    rng = np.random.default_rng(12)
+    spec.u = (1e-12 * rng.standard_normal(spec.u.shape)).astype(np.float32)
+    g, o = pair(spec, demag=False)
+    assert field_err(g.eval_accel(), o.acceleration(o.m, o.u, 0.0)) < FIELD_TOL
+    for s in range(2):
+        assert field_err(g.eval_heff(s, mmx.T_MEL), o.field_terms(s, terms=oc.T_MEL)[oc.T_MEL]) < FIELD_TOL
+    g.destroy()
