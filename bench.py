@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s of the Dormand-Prince RK45 LLG step with FFT demag on one B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mmx|reference] [--config c4]
+
+A "step" is one pass of the whole hot path: one DP45 step (6 effective-field evaluations with
+the full demag convolution, torque, stage combinations, error norm, controller) of BASELINE.json
+configs[3] (256x256x64 cells, padded FFT 512x512x128, fp32) -- the configuration the metric is
+quoted on -- at a fixed step size with forced acceptance ("Measurement").  One JSON
+line is printed by rank 0.  N > 1 runs N independent replicas (the path does not shard: DESIGN.md
+"Multi-GPU"), one process per GPU, timed as the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as wl  # noqa: E402
+
+METRIC = "cell-updates/s (RK45 LLG w/ demag)"
+UNIT = "cell-updates/s"
+DT = {"c1": 1e-13, "c2": 2e-14, "c3": 5e-15, "c4": 1e-13, "c5": 5e-15}
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
+# committed `ncu --set full` capture (profiles/, see the .md beside it); None until captured.
+NCU_TRAFFIC_BYTES = {"demag_inner": None}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def algorithmic_bytes(spec):
+    """Algorithmic HBM bytes per launch of every kernel category:
+    a pruned pass reads only non-zero input and writes only kept output."""
+    nx, ny, nz = spec.grid
+    N = nx * ny * nz
+    S = spec.S
+    def pad(n, p):
+        if p > 0:
+            return n
+        if n == 1:
+            return 1
+        q = 1
+        while q < n:
+            q *= 2
+        return 2 * q
+    px, py, pz = max(2, pad(nx, spec.pbc[0])), pad(ny, spec.pbc[1]), pad(nz, spec.pbc[2])
+    xc = px // 2 + 1
+    spec1 = 3 * nz * ny * xc * 8
+    spec2 = 3 * nz * py * xc * 8
+    ky, kz = (py // 2 + 1 if py > 1 else 1), (pz // 2 + 1 if pz > 1 else 1)
+    three_d = nz > 1
+    out = {
+        "demag_x_fwd": 12 * N * S + spec1,
+        "demag_x_inv": spec1 + 12 * N,
+        "demag_mid_fwd": spec1 + spec2,
+        "demag_mid_inv": spec2 + spec1,
+        "demag_inner": (2 * spec2 + 6 * kz * ky * xc * 4) if three_d else (2 * spec1 + 4 * ky * xc * 4),
+        # DP45: evaluation i = 1..5 moves (5 + i) fields, the last one 9: 49 fields of 12 N bytes / 6 launches
+        "local": 12 * N * S * 49 / 6.0,
+        "combine": 12 * N * S * 3,
+    }
+    return out
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 8:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out["sm_mhz"] = float(np.median(sm))
+            out["sm_max_mhz"] = float(max(mx))
+            out["samples"] = len(sm)
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def oracle_sample_grid(name, total_steps):
+    """Bounded sample of the workload for the CPU oracle: a box of the same shape, cell size,
+    material and seeded state recipe with fewer cells, sized so `total_steps` DP45 steps end
+    within a few minutes on the host cores."""
+    if name != "c4":
+        return {"c1": (64, 16, 1), "c2": (128, 128, 1), "c3": (256, 64, 1), "c5": (256, 64, 1)}[name]
+    if total_steps <= 3:
+        return (128, 128, 32)
+    if total_steps <= 60:
+        return (64, 64, 16)
+    return (32, 32, 8)
+
+
+def time_oracle(name, grid, steps, warmup):
+    """The oracle as it stands (never tuned), fixed-step DP45, wall clock on the host cores."""
+    from oracle.world import World as OracleWorld
+    spec = wl.make(name, grid)
+    o = OracleWorld(spec)
+    o.step_dp45_fixed(DT[name], max(warmup, 1))  # also builds its demag kernel (untimed setup)
+    t0 = time.perf_counter()
+    o.step_dp45_fixed(DT[name], steps)
+    dt = time.perf_counter() - t0
+    cells = grid[0] * grid[1] * grid[2]
+    return cells * steps / dt, dt / steps
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    grid = oracle_sample_grid(args.config, args.steps + args.warmup)
+    value, s_per_step = time_oracle(args.config, grid, args.steps, args.warmup)
+    cores = len(os.sched_getaffinity(0))
+    sample = "oracle fp64 DP45 fixed-step on a %dx%dx%d box of the %s recipe (bounded sample)" % (*grid, args.config)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * s_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": "%s sample %dx%dx%d" % (args.config, *grid)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_mmx(args, rank, local_rank, world_size):
+    import torch
+
+    import paper_2411_18194_b200 as mmx
+    from paper_2411_18194_b200 import build as b
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libmmx has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world_size > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        b.build()
+    if dist is not None:
+        dist.barrier()
+
+    name = args.config
+    spec = wl.make(name)                      # every rank: an independent replica, same recipe
+    if world_size > 1:
+        spec = wl.make(name, seed=1000 + int(name[1]) + 100 * rank)
+    N = spec.ncells
+    stream = torch.cuda.current_stream()
+    g = mmx.World.from_spec(spec, stream=stream.cuda_stream)
+    dt = DT[name]
+    K, W = args.steps, max(args.warmup, 3)
+
+    def steps(n):
+        return g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=n)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    steps(W)
+    clocks = ClockSampler(local_rank) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    st = steps(K)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop() if clocks else None
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = N * K * world_size / (ms * 1e-3)
+    launches = int(st["launches"])
+
+    # ---- roofline of the dominant kernel: CUDA events around every launch, on the launching stream
+    g.profile_enable(True)
+    steps(K)
+    prof = g.profile_read()
+    g.profile_enable(False)
+    alg = algorithmic_bytes(spec)
+    total_prof_ms = sum(v[0] for v in prof.values())
+    dom = max((k for k in prof if k in alg and prof[k][1] > 0), key=lambda k: prof[k][0])
+    peak, peak_src = measured_peaks()
+    dom_ms = prof[dom][0] / prof[dom][1]
+    achieved = alg[dom] / (dom_ms * 1e-3) / 1e9
+    kernels = {k: {"ms_per_launch": v[0] / v[1], "launches_per_step": v[1] / K, "share": v[0] / total_prof_ms,
+                   "GBs": (alg[k] / (v[0] / v[1] * 1e-3) / 1e9) if k in alg else None}
+               for k, v in prof.items() if v[1] > 0}
+    step_bytes = sum(alg[k] * prof[k][1] / K for k in prof if k in alg and prof[k][1] > 0)
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(dom), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg[dom], "ms_per_launch": dom_ms,
+                "step_algorithmic_bytes": step_bytes,
+                "step_frac_of_peak": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
+                "step_frac_of_8TBs": step_bytes / (ms / K * 1e-3) / 8e12,
+                "kernels": kernels}
+
+    # ---- end to end through the C-ABI with HOST buffers: H2D of m, one step, D2H of m, every step
+    Ke = min(K, 5)
+    hin = torch.from_numpy(np.ascontiguousarray(spec.m[0])).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    def e2e_step():
+        for s in range(spec.S):
+            g.set_state(mmx.F_M0 + s, hin if s == 0 else torch.from_numpy(spec.m[s]))
+        g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=1)
+        g.get_state(mmx.F_M0, hout)
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        e2e_step()
+    torch.cuda.synchronize()
+    te = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([te], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        te = float(t.item())
+    e2e = {"value": N * Ke * world_size / te, "unit": UNIT, "h2d_bytes_per_step": 12 * N * spec.S,
+           "d2h_bytes_per_step": 12 * N, "steps": Ke,
+           "note": "set_state(host) + 1 DP45 step (7 evaluations: k1 is recomputed after set_state) + get_state(host)"}
+
+    # ---- separate adaptive run: accepted / rejected counts (not the timed figure)
+    ad = g.step_rk45(method=mmx.DP45, tol=1e-5, dt0=dt, nsteps=10)
+    adaptive = {"accepted": ad["accepted"], "rejected": ad["rejected"], "dt": ad["dt"]}
+    dev_bytes = g.device_bytes()
+    g.destroy()
+
+    cpu = None
+    if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
+        grid = oracle_sample_grid(name, 1)
+        v, s_step = time_oracle(name, grid, 1, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
+               "sample": "1 fixed-step DP45 step of the fp64 numpy oracle on a %dx%dx%d box of the %s recipe "
+                         "(%.1f s)" % (*grid, name, s_step)}
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "%s %dx%dx%d DP45 fixed dt=%g, demag+exchange" % (name, *spec.grid, dt),
+                       "cells": N, "field_evals_per_s": value * 6,
+                       "l2": "working set %.2f GB >> 126 MB L2, no flush needed" % (dev_bytes / 1e9),
+                       "parallelism": "replicas x%d" % world_size},
+            "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "cpu_baseline": cpu, "adaptive": adaptive,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="mmx", choices=["mmx", "reference"])
+    ap.add_argument("--config", default="c4", choices=list(DT))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world_size = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if world_size != args.gpus and world_size == 1 and args.gpus > 1:
+        raise SystemExit("launch with torch.distributed.run --nproc-per-node %d" % args.gpus)
+    run_mmx(args, rank, local_rank, world_size)
+
+
+if __name__ == "__main__":
+    main()
