@@ -287,7 +287,7 @@ int mmx_demag_plan_sizes(mmx_world* w) {
     if (P[a] > 2048) return mmx_fail(MMX_EINVAL, "transform length %d on axis %d exceeds 2048", P[a], a);
   d.px = P[0]; d.py = P[1]; d.pz = P[2];
   d.xc = d.px / 2 + 1;
-  d.xp = (d.xc + 3) & ~3;
+  d.xp = (d.xc + 15) & ~15;  // rows start on 128-byte boundaries
   d.ky = d.py > 1 ? d.py / 2 + 1 : 1;
   d.kz = d.pz > 1 ? d.pz / 2 + 1 : 1;
   return MMX_OK;
@@ -330,7 +330,12 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ProfScope ps(w, PK_MID_FWD);                                                           \
     k_mid<PP, -1><<<g, block_for(PP), sm, st>>>(ma);                                      \
   }
-    MMX_SWITCH_P(d.py, 2, CALL_MF)
+    if (mmx_mid_col_ok(d.py, d.ny)) {
+      if (int rc = mmx_mid_col_launch(w, d.py, -1, d.spec1, d.spec2, d.ny, d.py, ma.in_outer, ma.out_outer,
+                                      3 * d.nz, d.tw[1])) return rc;
+    } else {
+      MMX_SWITCH_P(d.py, 2, CALL_MF)
+    }
     w->launches++;
   }
 
@@ -365,7 +370,16 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ProfScope ps(w, PK_INNER);                                                             \
     k_inner<PP><<<g, block_for(PP), sm, st>>>(ia);                                        \
   }
-    MMX_SWITCH_P(Pin, 1, CALL_IN)
+    if (mmx_inner_col_ok(d, Pin, ia.n_valid)) {
+      InnerColLaunch L;
+      L.spec = ia.spec; L.tw = ia.tw; L.n_valid = ia.n_valid; L.p_outer = ia.p_outer; L.n_outer = nouter;
+      L.line_stride = ia.line_stride; L.comp_stride = ia.comp_stride; L.outer_stride = ia.outer_stride;
+      L.k_inner_stride = ia.k_inner_stride; L.k_outer_stride = ia.k_outer_stride; L.k_comp_stride = ia.k_comp_stride;
+      L.odd_inner = ia.odd_inner; L.odd_outer = ia.odd_outer;
+      if (int rc = mmx_inner_col_launch(w, L)) return rc;
+    } else {
+      MMX_SWITCH_P(Pin, 1, CALL_IN)
+    }
     w->launches++;
   }
 
@@ -383,7 +397,12 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ProfScope ps(w, PK_MID_INV);                                                           \
     k_mid<PP, +1><<<g, block_for(PP), sm, st>>>(ma);                                      \
   }
-    MMX_SWITCH_P(d.py, 2, CALL_MI)
+    if (mmx_mid_col_ok(d.py, d.ny)) {
+      if (int rc = mmx_mid_col_launch(w, d.py, +1, d.spec2, d.spec1, d.py, d.ny, ma.in_outer, ma.out_outer,
+                                      3 * d.nz, d.tw[1])) return rc;
+    } else {
+      MMX_SWITCH_P(d.py, 2, CALL_MI)
+    }
     w->launches++;
   }
 

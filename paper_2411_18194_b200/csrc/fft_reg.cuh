@@ -1,0 +1,118 @@
+// fft_reg.cuh -- register-resident radix-4/8/16 DFT butterflies, fp32, for the "column" FFT
+// kernels of demag.cu (one thread owns R points of a line, R threads own a line of R*R
+// points, the only exchange between the two radix-R stages goes through shared memory).
+//
+// A transform of length P = 2 R^2 along a strided axis is split by one radix-2
+// decimation-in-frequency step into its even and odd outputs,
+//     X[2k]   = DFT_H( x[n] + x[n+H] )[k]
+//     X[2k+1] = DFT_H( (x[n] - x[n+H]) w_P^n )[k]            H = P/2 = R^2, w_P = exp(-2 pi i/P)
+// and the zero padding of the demag convolution (x[n] = 0 for n >= H on an open axis) makes
+// the butterfly free: both halves start from the same H loaded points.  The inverse uses the
+// mirrored decimation-in-time step and needs only the first H outputs,
+//     x[n] = IDFT_H(X[2k])[n] + conj(w_P^n) IDFT_H(X[2k+1])[n].
+// Each H-point transform is two radix-R stages:
+//     n = j + R u, k = a + R b:   X[a + R b] = sum_j w_R^(j b) [ w_H^(j a) sum_u x[j + R u] w_R^(u a) ]
+// Twiddles come from a table tw[q] = exp(-2 pi i q / P) rounded from fp64 (never products of
+// fp32 twiddles), so w_H^(j a) = tw[2 j a] and w_P^n = tw[n].
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mmxreg {
+
+#define MMX_DI __device__ __forceinline__
+
+MMX_DI float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+MMX_DI float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+MMX_DI float2 cmul(float2 a, float2 b) {
+  return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+// a * conj(b)
+MMX_DI float2 cmulc(float2 a, float2 b) {
+  return make_float2(fmaf(a.x, b.x, a.y * b.y), fmaf(a.y, b.x, -a.x * b.y));
+}
+// a * w (DIR < 0, forward) or a * conj(w) (DIR > 0, inverse), w a forward twiddle
+template <int DIR>
+MMX_DI float2 ctw(float2 a, float2 w) {
+  return DIR < 0 ? cmul(a, w) : cmulc(a, w);
+}
+// multiply by DIR * i
+template <int DIR>
+MMX_DI float2 mul_i(float2 a) {
+  return DIR < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+}
+// multiply by (c + i DIR s): exp(DIR i theta) with c = cos theta, s = sin theta
+template <int DIR>
+MMX_DI float2 rot(float2 a, float c, float s) {
+  const float d = DIR < 0 ? -s : s;
+  return make_float2(fmaf(a.x, c, -a.y * d), fmaf(a.x, d, a.y * c));
+}
+
+template <int DIR>
+MMX_DI void dft4(float2& x0, float2& x1, float2& x2, float2& x3) {
+  const float2 a = cadd(x0, x2), b = csub(x0, x2);
+  const float2 c = cadd(x1, x3), d = mul_i<DIR>(csub(x1, x3));
+  x0 = cadd(a, c);
+  x1 = cadd(b, d);
+  x2 = csub(a, c);
+  x3 = csub(b, d);
+}
+
+// X[q] = sum_r v[r] exp(DIR 2 pi i q r / R), natural order in and out
+template <int R, int DIR>
+struct Dft;
+
+template <int DIR>
+struct Dft<4, DIR> {
+  static MMX_DI void run(float2* v) { dft4<DIR>(v[0], v[1], v[2], v[3]); }
+};
+
+template <int DIR>
+struct Dft<8, DIR> {
+  static MMX_DI void run(float2* v) {
+    const float h = 0.70710678118654752440f;
+    float2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6];
+    float2 o0 = v[1], o1 = v[3], o2 = v[5], o3 = v[7];
+    dft4<DIR>(e0, e1, e2, e3);
+    dft4<DIR>(o0, o1, o2, o3);
+    const float2 t1 = rot<DIR>(o1, h, h);
+    const float2 t2 = mul_i<DIR>(o2);
+    const float2 t3 = rot<DIR>(o3, -h, h);
+    v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+    v[1] = cadd(e1, t1); v[5] = csub(e1, t1);
+    v[2] = cadd(e2, t2); v[6] = csub(e2, t2);
+    v[3] = cadd(e3, t3); v[7] = csub(e3, t3);
+  }
+};
+
+template <int DIR>
+struct Dft<16, DIR> {
+  // 16 = 4 x 4:  n = 4 n1 + n2,  k = k1 + 4 k2
+  //   X[k1 + 4 k2] = sum_n2 w4^(n2 k2) [ w16^(n2 k1) sum_n1 v[4 n1 + n2] w4^(n1 k1) ]
+  static MMX_DI void run(float2* v) {
+    const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;
+    const float h = 0.70710678118654752440f;
+    float2 t[4][4];  // t[n2][k1]
+#pragma unroll
+    for (int n2 = 0; n2 < 4; ++n2) {
+      t[n2][0] = v[n2]; t[n2][1] = v[4 + n2]; t[n2][2] = v[8 + n2]; t[n2][3] = v[12 + n2];
+      dft4<DIR>(t[n2][0], t[n2][1], t[n2][2], t[n2][3]);
+    }
+    // w16^(n2 k1)
+    t[1][1] = rot<DIR>(t[1][1], c1, s1);
+    t[1][2] = rot<DIR>(t[1][2], h, h);
+    t[1][3] = rot<DIR>(t[1][3], s1, c1);
+    t[2][1] = rot<DIR>(t[2][1], h, h);
+    t[2][2] = mul_i<DIR>(t[2][2]);
+    t[2][3] = rot<DIR>(t[2][3], -h, h);
+    t[3][1] = rot<DIR>(t[3][1], s1, c1);
+    t[3][2] = rot<DIR>(t[3][2], -h, h);
+    t[3][3] = rot<DIR>(t[3][3], -c1, -s1);  // w16^9 = -w16^1
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) {
+      dft4<DIR>(t[0][k1], t[1][k1], t[2][k1], t[3][k1]);  // index k2 now lives in the first slot
+      v[k1] = t[0][k1]; v[k1 + 4] = t[1][k1]; v[k1 + 8] = t[2][k1]; v[k1 + 12] = t[3][k1];
+    }
+  }
+};
+
+}  // namespace mmxreg

@@ -211,6 +211,21 @@ int mmx_kernel_spectrum(const int grid[3], const int pbc[3], const int P[3], int
 int mmx_demag_plan_sizes(mmx_world* w);
 int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout);
 
+// demag_col.cu: register-resident column passes (fast path for P = 2 R^2 on a pruned axis)
+struct InnerColLaunch {
+  float2* spec;
+  const float2* tw;
+  int n_valid, p_outer, n_outer;
+  size_t line_stride, comp_stride, outer_stride;
+  size_t k_inner_stride, k_outer_stride, k_comp_stride;
+  unsigned odd_inner, odd_outer;
+};
+bool mmx_inner_col_ok(const DemagPlan& d, int P, int n_valid);
+int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L);
+bool mmx_mid_col_ok(int P, int n);
+int mmx_mid_col_launch(mmx_world* w, int P, int dir, const float2* in, float2* out, int n_in, int n_out,
+                       size_t in_outer, size_t out_outer, int nslab, const float2* tw);
+
 // local.cu
 int mmx_local_launch(mmx_world* w, const LocalArgs& a);
 int mmx_combine_launch(mmx_world* w, const float* const y0[2], const float* const k1[2],
