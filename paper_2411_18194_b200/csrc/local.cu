@@ -245,6 +245,254 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
   if (a.do_tq) block_max_to(tqv, &ctrl->tq_bits);
 }
 
+// ---- fast path: one region (uniform material, Ms > 0), Nx a multiple of 4 ------------------------
+// One thread owns four x-consecutive cells; every global access is a float4 (centre, y/z
+// neighbours, B_demag, y0, k_j, outputs) except the two x-edge neighbours.  Same arithmetic,
+// term by term, as k_local.
+struct Q3 {  // four cells of a 3-vector field
+  V3 c[4];
+};
+__device__ __forceinline__ Q3 ldq(const float* p, size_t N, size_t i) {
+  const float4 x = *reinterpret_cast<const float4*>(p + i);
+  const float4 y = *reinterpret_cast<const float4*>(p + N + i);
+  const float4 z = *reinterpret_cast<const float4*>(p + 2 * N + i);
+  Q3 q;
+  q.c[0] = v3(x.x, y.x, z.x); q.c[1] = v3(x.y, y.y, z.y); q.c[2] = v3(x.z, y.z, z.z); q.c[3] = v3(x.w, y.w, z.w);
+  return q;
+}
+__device__ __forceinline__ void stq(float* p, size_t N, size_t i, const Q3& q) {
+  *reinterpret_cast<float4*>(p + i) = make_float4(q.c[0].x, q.c[1].x, q.c[2].x, q.c[3].x);
+  *reinterpret_cast<float4*>(p + N + i) = make_float4(q.c[0].y, q.c[1].y, q.c[2].y, q.c[3].y);
+  *reinterpret_cast<float4*>(p + 2 * N + i) = make_float4(q.c[0].z, q.c[1].z, q.c[2].z, q.c[3].z);
+}
+
+#ifndef MMX_L4_MINB
+#define MMX_L4_MINB 2
+#endif
+// NP = n_prev, the number of earlier k_j of the RK combination; MODE bit 0: form the next stage
+// state, bit 1: form the embedded error
+template <int S, int NP, int MODE>
+__global__ void __launch_bounds__(256, MMX_L4_MINB) k_local4(LocalArgs a) {
+  MmxCtrl* ctrl = a.ctrl;
+  if (!ctrl->active) return;
+  const int sel = ctrl->sel;
+  const size_t N = (size_t)a.nx * a.ny * a.nz;
+  const unsigned gpr = a.nx >> 2;  // groups per row
+  const unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned rows = (unsigned)a.ny * a.nz;
+  const float* yin = a.yin[sel];
+  float errv = 0.f, tqv = 0.f;
+  bool bad = false;
+  if (g < gpr * rows) {
+    const unsigned row = g / gpr;
+    const int ix = (int)(g - row * gpr) << 2;
+    const int iz = (int)(row / (unsigned)a.ny), iy = (int)(row - (unsigned)iz * a.ny);
+    const size_t i = (size_t)row * a.nx + ix;
+    // neighbour offsets (in elements) along y and z; valid flags
+    long long off[6];
+    bool val[6];
+    {
+      const bool xm = ix > 0, xp = ix + 4 < a.nx;
+      val[1] = xm || a.per[0]; off[1] = xm ? -1 : (long long)a.nx - 1;
+      val[0] = xp || a.per[0]; off[0] = xp ? 4 : 4 - (long long)a.nx;
+      const bool ym = iy > 0, yp = iy + 1 < a.ny;
+      val[3] = ym || (a.per[1] && a.ny > 1); off[3] = ym ? -(long long)a.nx : (long long)(a.ny - 1) * a.nx;
+      val[2] = yp || (a.per[1] && a.ny > 1); off[2] = yp ? (long long)a.nx : -(long long)(a.ny - 1) * a.nx;
+      const long long pl = (long long)a.nx * a.ny;
+      const bool zm = iz > 0, zp = iz + 1 < a.nz;
+      val[5] = zm || (a.per[2] && a.nz > 1); off[5] = zm ? -pl : (long long)(a.nz - 1) * pl;
+      val[4] = zp || (a.per[2] && a.nz > 1); off[4] = zp ? pl : -(long long)(a.nz - 1) * pl;
+    }
+    Q3 mc[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) mc[s] = ldq(yin + (size_t)s * 3 * N, N, i);
+
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      if (a.heff_out || a.tau_out) {
+        if (s != a.heff_s) continue;
+      }
+      const int o = S == 2 ? 1 - s : s;
+      // RK epilogue inputs first (independent of the field): ys = y0 + sum_j ca_j k_j, er = sum_j ce_j k_j
+      constexpr bool comb = (MODE & 1) != 0, doerr = (MODE & 2) != 0;
+      const bool epi = !a.heff_out && !a.tau_out;
+      const float* ca = ctrl->ca[a.combine_row];
+      const float* ce = ctrl->ce;
+      Q3 ys, er;
+      if (MODE != 0 && epi) {
+        if (comb) ys = ldq(a.y0[sel] + (size_t)s * 3 * N, N, i);
+        if (doerr) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) er.c[e] = v3(0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int j = 0; j < NP; ++j) {
+          const float cj = comb ? ca[j] : 0.f;
+          const float ej = doerr ? ce[j] : 0.f;
+          if (cj != 0.f || ej != 0.f) {
+            const Q3 kj = ldq(a.kprev[sel][j] + (size_t)s * 3 * N, N, i);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              if (comb) ys.c[e] = fma3(cj, kj.c[e], ys.c[e]);
+              if (doerr) er.c[e] = fma3(ej, kj.c[e], er.c[e]);
+            }
+          }
+        }
+      }
+      const float* P = a.mat + (size_t)s * MMX_MATW;
+      const float iMs = P[MP_INVMS];
+      const float* ms_ = yin + (size_t)s * 3 * N;
+      const float* mo_ = yin + (size_t)o * 3 * N;
+      const bool use12 = S == 2 && (a.terms & (MMX_T_A12 | MMX_T_DMI_INTER));
+      Q3 B, dm;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { B.c[e] = v3(0.f, 0.f, 0.f); dm.c[e] = v3(0.f, 0.f, 0.f); }
+      const float Ac = P[MP_A], Dc = P[MP_D], zlb = P[MP_ZLB];
+#pragma unroll
+      for (int q = 0; q < 6; ++q) {
+        const int axis = q >> 1;
+        const float d = (q & 1) ? -1.f : 1.f;
+        // neighbour values of the four cells along direction q (own and partner sublattice)
+        Q3 mn = mc[s], on = mc[o];
+        bool v[4] = {val[q], val[q], val[q], val[q]};
+        if (axis == 0) {
+          // interior cells take their x neighbour from the thread's own registers
+          // (loads are unconditional -- an absent neighbour reads the thread's own cell -- so that
+          // the compiler can issue all of them before the first use)
+          const size_t ei = val[q] ? (size_t)((long long)i + off[q]) : i;
+          const V3 edge = ld3(ms_, N, ei);
+          V3 oedge = edge;
+          if (use12) oedge = ld3(mo_, N, ei);
+          if (q == 0) {
+            mn.c[0] = mc[s].c[1]; mn.c[1] = mc[s].c[2]; mn.c[2] = mc[s].c[3]; mn.c[3] = edge;
+            on.c[0] = mc[o].c[1]; on.c[1] = mc[o].c[2]; on.c[2] = mc[o].c[3]; on.c[3] = oedge;
+            v[0] = v[1] = v[2] = true;
+          } else {
+            mn.c[3] = mc[s].c[2]; mn.c[2] = mc[s].c[1]; mn.c[1] = mc[s].c[0]; mn.c[0] = edge;
+            on.c[3] = mc[o].c[2]; on.c[2] = mc[o].c[1]; on.c[1] = mc[o].c[0]; on.c[0] = oedge;
+            v[1] = v[2] = v[3] = true;
+          }
+        } else {
+          const size_t ni = val[q] ? (size_t)((long long)i + off[q]) : i;
+          mn = ldq(ms_, N, ni);
+          if (use12) on = ldq(mo_, N, ni);
+        }
+        const float wex = 2.f * harm(Ac, Ac) * iMs * a.inv_h2[axis];
+        const float wd = harm(Dc, Dc) * iMs * a.inv_h[axis] * d;
+        const float w12 = a.A12 * iMs * a.inv_h2[axis];
+        const float wdi = a.Dinter * iMs * a.inv_h[axis] * d;
+        const float wu = zlb * a.J[axis] * 0.5f * a.inv_h[axis] * d;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          if (v[e]) {
+            if (a.terms & MMX_T_EXCH) B.c[e] = fma3(wex, mn.c[e] - mc[s].c[e], B.c[e]);
+            if (axis < 2 && (a.terms & MMX_T_DMI)) {
+              if (axis == 0) { B.c[e].x = fmaf(wd, mn.c[e].z, B.c[e].x); B.c[e].z = fmaf(-wd, mn.c[e].x, B.c[e].z); }
+              else { B.c[e].y = fmaf(wd, mn.c[e].z, B.c[e].y); B.c[e].z = fmaf(-wd, mn.c[e].y, B.c[e].z); }
+            }
+            if (S == 2) {
+              if (a.terms & MMX_T_A12) B.c[e] = fma3(w12, on.c[e] - mc[o].c[e], B.c[e]);
+              if (axis < 2 && (a.terms & MMX_T_DMI_INTER)) {
+                if (axis == 0) { B.c[e].x = fmaf(wdi, on.c[e].z, B.c[e].x); B.c[e].z = fmaf(-wdi, on.c[e].x, B.c[e].z); }
+                else { B.c[e].y = fmaf(wdi, on.c[e].z, B.c[e].y); B.c[e].z = fmaf(-wdi, on.c[e].y, B.c[e].z); }
+              }
+            }
+          }
+          if (a.has_J) dm.c[e] = fma3(wu, v[e] ? mn.c[e] : mc[s].c[e], dm.c[e]);
+        }
+      }
+      Q3 bd, tau;
+      const bool use_bd = (a.terms & MMX_T_DEMAG) && a.bdemag;
+      if (use_bd) bd = ldq(a.bdemag, N, i);
+      float eps[6][4];
+      const bool use_mel = (a.terms & MMX_T_MEL) && a.strain;
+      if (use_mel) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+          const float4 t = *reinterpret_cast<const float4*>(a.strain + (size_t)c * N + i);
+          eps[c][0] = t.x; eps[c][1] = t.y; eps[c][2] = t.z; eps[c][3] = t.w;
+        }
+      }
+      const float alpha = P[MP_ALPHA], llg = P[MP_LLG], xi = P[MP_XI];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const V3 m = mc[s].c[e];
+        V3 Bc = B.c[e];
+        if (S == 2 && (a.terms & MMX_T_A0)) Bc = fma3(a.a0pref * iMs, mc[o].c[e], Bc);
+        if (a.terms & MMX_T_ANIS_U) {
+          const V3 u = v3(P[MP_UX], P[MP_UY], P[MP_UZ]);
+          Bc = fma3(P[MP_KU2] * dot(u, m), u, Bc);
+        }
+        if ((a.terms & MMX_T_ANIS_C) && P[MP_KC2] != 0.f) {
+          const V3 c1 = v3(P[MP_C1X], P[MP_C1Y], P[MP_C1Z]);
+          const V3 c2 = v3(P[MP_C2X], P[MP_C2Y], P[MP_C2Z]);
+          const V3 c3 = v3(P[MP_C3X], P[MP_C3Y], P[MP_C3Z]);
+          const float a1 = dot(c1, m), a2 = dot(c2, m), a3 = dot(c3, m);
+          const float k = -P[MP_KC2];
+          Bc = fma3(k * a1 * (a2 * a2 + a3 * a3), c1, Bc);
+          Bc = fma3(k * a2 * (a3 * a3 + a1 * a1), c2, Bc);
+          Bc = fma3(k * a3 * (a1 * a1 + a2 * a2), c3, Bc);
+        }
+        if (a.terms & MMX_T_ZEEMAN) Bc = Bc + v3(a.bext[0], a.bext[1], a.bext[2]);
+        if (use_bd) Bc = Bc + bd.c[e];
+        if (use_mel) {
+          const float p1 = -P[MP_MEL1], p2 = -P[MP_MEL2];
+          Bc.x += p1 * eps[0][e] * m.x + p2 * (eps[3][e] * m.y + eps[4][e] * m.z);
+          Bc.y += p1 * eps[1][e] * m.y + p2 * (eps[3][e] * m.x + eps[5][e] * m.z);
+          Bc.z += p1 * eps[2][e] * m.z + p2 * (eps[4][e] * m.x + eps[5][e] * m.y);
+        }
+        B.c[e] = Bc;
+        const V3 mxB = cross(m, Bc);
+        const V3 mxmxB = cross(m, mxB);
+        V3 t = (-llg) * fma3(alpha, mxmxB, mxB);
+        if (a.has_J) {
+          const V3 mxa = cross(m, dm.c[e]);
+          const V3 mxmxa = cross(m, mxa);
+          const float inv = -1.f / (1.f + alpha * alpha);
+          t = fma3(inv * (1.f + xi * alpha), mxmxa, t);
+          t = fma3(inv * (xi - alpha), mxa, t);
+        }
+        tau.c[e] = t;
+      }
+      if (a.heff_out) { stq(a.heff_out, N, i, B); continue; }
+      if (a.tau_out) { stq(a.tau_out, N, i, tau); continue; }
+      stq(a.kout[sel] + (size_t)s * 3 * N, N, i, tau);
+      if (a.do_tq) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float t2 = dot(tau.c[e], tau.c[e]);
+          tqv = fmaxf(tqv, sqrtf(t2));
+          bad |= !(t2 == t2);
+        }
+      }
+      if (comb) {
+        const float cs = ca[a.stage];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          V3 yy = fma3(cs, tau.c[e], ys.c[e]);
+          const float n2 = dot(yy, yy);
+          if (n2 > 0.f) yy = (1.f / sqrtf(n2)) * yy;
+          ys.c[e] = yy;
+        }
+        stq(a.ynext[sel] + (size_t)s * 3 * N, N, i, ys);
+      }
+      if (doerr) {
+        const float es = ce[a.stage];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const V3 ee = fma3(es, tau.c[e], er.c[e]);
+          const float e2 = dot(ee, ee);
+          errv = fmaxf(errv, sqrtf(e2));
+          bad |= !(e2 == e2);
+        }
+      }
+    }
+  }
+  if (bad) errv = tqv = __int_as_float(0x7fc00000);
+  if (a.do_err) block_max_to(errv, &ctrl->err_bits);
+  if (a.do_tq) block_max_to(tqv, &ctrl->tq_bits);
+}
+
 // y_next = project(y0 + ca[row][0] * k1) for all vectors (m normalised, u and v not)
 __global__ void __launch_bounds__(256) k_combine1(const float* y0a, const float* y0b, const float* k1a,
                                                   const float* k1b, float* yna, float* ynb, int row, int S,
@@ -360,7 +608,22 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   const unsigned blocks = (unsigned)((N + 255) / 256);
   const bool reg = w->nreg > 1;
   ProfScope ps(w, PK_LOCAL);
-  if (w->S == 1) {
+  bool uniform = !reg && (w->grid[0] % 4) == 0;
+  for (int s = 0; s < w->S && uniform; ++s) uniform = w->mats[(size_t)s * w->nreg].Ms > 0;
+  if (uniform) {
+    const unsigned b4 = (unsigned)((N / 4 + 255) / 256);
+    const int mode = (a.ynext[0] ? 1 : 0) | (a.do_err ? 2 : 0);
+#define MMX_L4(S_, NP_)                                                    \
+  case NP_:                                                                \
+    if (mode == 0) k_local4<S_, 0, 0><<<b4, 256, 0, w->stream>>>(a);       \
+    else if (mode == 1) k_local4<S_, NP_, 1><<<b4, 256, 0, w->stream>>>(a); \
+    else if (mode == 2) k_local4<S_, NP_, 2><<<b4, 256, 0, w->stream>>>(a); \
+    else k_local4<S_, NP_, 3><<<b4, 256, 0, w->stream>>>(a);               \
+    break;
+#define MMX_L4_ALL(S_) switch (a.n_prev) { MMX_L4(S_, 0) MMX_L4(S_, 1) MMX_L4(S_, 2) MMX_L4(S_, 3) MMX_L4(S_, 4) \
+    MMX_L4(S_, 5) MMX_L4(S_, 6) MMX_L4(S_, 7) default: return mmx_fail(MMX_EINVAL, "n_prev %d out of range", a.n_prev); }
+    if (w->S == 1) { MMX_L4_ALL(1) } else { MMX_L4_ALL(2) }
+  } else if (w->S == 1) {
     if (reg) k_local<1, true><<<blocks, 256, 0, w->stream>>>(a);
     else k_local<1, false><<<blocks, 256, 0, w->stream>>>(a);
   } else {
