@@ -499,6 +499,13 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
   w->nvec = w->S;
   w->N = (size_t)grid[0] * grid[1] * grid[2];
   w->stream = (cudaStream_t)cuda_stream;
+  {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    w->sm_count = 148;
+    cudaDeviceGetAttribute(&w->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (w->sm_count <= 0) w->sm_count = 148;
+  }
   w->nreg = 1;
   w->d_reg = nullptr;
   w->mats.resize(w->S);

@@ -313,7 +313,12 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ProfScope ps(w, PK_X_FWD);                                                             \
     k_x_fwd<PP><<<(rows + 2 * L - 1) / (2 * L), block_for(PP), sm, st>>>(xa);             \
   }
-  MMX_SWITCH_P(d.px, 2, CALL_XF)
+  const bool xwarp = mmx_x_warp_ok(w);
+  if (xwarp) {
+    if (int rc = mmx_x_warp_launch(w, -1, yin, bout)) return rc;
+  } else {
+    MMX_SWITCH_P(d.px, 2, CALL_XF)
+  }
   w->launches++;
 
   if (three_d && d.py > 1) {
@@ -414,7 +419,11 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ProfScope ps(w, PK_X_INV);                                                             \
     k_x_inv<PP><<<(rows + 2 * L - 1) / (2 * L), block_for(PP), sm, st>>>(xa);             \
   }
-  MMX_SWITCH_P(d.px, 2, CALL_XI)
+  if (xwarp) {
+    if (int rc = mmx_x_warp_launch(w, +1, yin, bout)) return rc;
+  } else {
+    MMX_SWITCH_P(d.px, 2, CALL_XI)
+  }
   w->launches++;
   MMX_CUDA(cudaGetLastError());
   return MMX_OK;

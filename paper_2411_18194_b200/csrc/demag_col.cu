@@ -20,6 +20,10 @@
 
 using namespace mmxreg;
 
+#ifndef MMX_MID_PERSISTENT
+#define MMX_MID_PERSISTENT 1
+#endif
+
 namespace {
 
 __device__ __forceinline__ void prefetch_l2(const void* p) {
@@ -268,6 +272,105 @@ __global__ void __launch_bounds__(2 * R * TILE, 2) k_mid_col(MidColArgs a) {
   }
 }
 
+// Persistent variant: one CTA per SM walks over the tiles and loads the points of its next tile
+// into registers before it transforms the current one, so that global loads are in flight
+// during the whole kernel (the non-persistent CTAs above alternate between a load phase and a
+// compute phase and leave HBM idle in between).
+template <int R, int TILE, int DIR>
+__global__ void __launch_bounds__(2 * R * TILE, 1) k_mid_colp(MidColArgs a) {
+  constexpr int H = R * R, P = 2 * H, T = 2 * R * TILE;
+  extern __shared__ float2 sm[];  // forward: [2][H][TILE]; inverse: [3][H][TILE]
+  __shared__ float2 stw[P];
+  if (a.gated && !a.ctrl->active) return;
+  const int t = threadIdx.x;
+  const int kxl = t % TILE, j = (t / TILE) % R, h = t / (TILE * R);
+  const int ntm = a.ntile_main * a.nslab;
+  const int nt = ntm + (a.nyq ? (a.nslab + TILE - 1) / TILE : 0);
+  for (int q = t; q < P; q += T) stw[q] = a.tw[q];
+  float2* ex = sm + (size_t)h * H * TILE + kxl;
+
+  auto locate = [&](int tile, int& kx, int& slab) -> bool {
+    bool ok;
+    if (tile < ntm) {
+      slab = tile / a.ntile_main; kx = (tile - slab * a.ntile_main) * TILE + kxl; ok = kx < a.xc_main;
+    } else {
+      kx = a.xc - 1; slab = (tile - ntm) * TILE + kxl; ok = slab < a.nslab;
+    }
+    if (!ok) { kx = 0; slab = 0; }
+    return ok;
+  };
+  auto load = [&](int tile, float2* v) {
+    int kx, slab;
+    const bool ok = locate(tile, kx, slab);
+    const float2* in = a.in + (size_t)slab * a.in_outer + kx;
+#pragma unroll
+    for (int u = 0; u < R; ++u) {
+      const int n = DIR < 0 ? j + R * u : 2 * (j + R * u) + h;
+      v[u] = (ok && n < a.n_in) ? in[(size_t)n * a.xp] : make_float2(0.f, 0.f);
+    }
+  };
+
+  float2 nxt[R];
+  int tile = blockIdx.x;
+  if (tile < nt) load(tile, nxt);
+  __syncthreads();  // stw
+  for (; tile < nt; tile += gridDim.x) {
+    float2 v[R];
+#pragma unroll
+    for (int u = 0; u < R; ++u) v[u] = nxt[u];
+    if (tile + (int)gridDim.x < nt) load(tile + gridDim.x, nxt);
+    int kx, slab;
+    const bool ok = locate(tile, kx, slab);
+    float2* out = a.out + (size_t)slab * a.out_outer + kx;
+    if (DIR < 0 && h) {
+#pragma unroll
+      for (int u = 0; u < R; ++u) v[u] = cmul(v[u], stw[j + R * u]);
+    }
+    Dft<R, DIR>::run(v);
+    ex[(0 * R + j) * TILE] = v[0];
+#pragma unroll
+    for (int q = 1; q < R; ++q) ex[(q * R + j) * TILE] = ctw<DIR>(v[q], stw[2 * j * q]);
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < R; ++q) v[q] = ex[(j * R + q) * TILE];
+    Dft<R, DIR>::run(v);
+    if (DIR < 0) {
+      if (ok) {
+#pragma unroll
+        for (int b = 0; b < R; ++b) out[(size_t)(2 * (j + R * b) + h) * a.xp] = v[b];
+      }
+    } else {
+      float2* sw = sm + (size_t)2 * H * TILE + kxl;
+      if (h) {
+#pragma unroll
+        for (int b = 0; b < R; ++b) v[b] = cmulc(v[b], stw[j + R * b]);
+#pragma unroll
+        for (int b = 0; b < R / 2; ++b) sw[(j + R * b) * TILE] = v[b];
+      } else {
+#pragma unroll
+        for (int b = R / 2; b < R; ++b) sw[(j + R * b) * TILE] = v[b];
+      }
+      __syncthreads();
+      if (h) {
+#pragma unroll
+        for (int b = R / 2; b < R; ++b) {
+          const int n = j + R * b;
+          const float2 o = cadd(v[b], sw[n * TILE]);
+          if (ok && n < a.n_out) out[(size_t)n * a.xp] = o;
+        }
+      } else {
+#pragma unroll
+        for (int b = 0; b < R / 2; ++b) {
+          const int n = j + R * b;
+          const float2 o = cadd(v[b], sw[n * TILE]);
+          if (ok && n < a.n_out) out[(size_t)n * a.xp] = o;
+        }
+      }
+    }
+    __syncthreads();  // exchange tiles are rewritten by the next iteration
+  }
+}
+
 template <typename Kern>
 int set_smem_col(Kern k, size_t bytes) {
   if (bytes > 48 * 1024) MMX_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
@@ -312,6 +415,17 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
   dim3 g(a.ntile_main + a.nyq, a.nslab);
   const size_t smem = sizeof(float2) * (dir < 0 ? 2 : 3) * R * R * TILE;
   ProfScope ps(w, dir < 0 ? PK_MID_FWD : PK_MID_INV);
+  const int ntiles = a.ntile_main * a.nslab + (a.nyq ? (a.nslab + TILE - 1) / TILE : 0);
+  if (MMX_MID_PERSISTENT && ntiles >= 4 * w->sm_count) {
+    if (dir < 0) {
+      if (int rc = set_smem_col(k_mid_colp<R, TILE, -1>, smem)) return rc;
+      k_mid_colp<R, TILE, -1><<<w->sm_count, 2 * R * TILE, smem, w->stream>>>(a);
+    } else {
+      if (int rc = set_smem_col(k_mid_colp<R, TILE, +1>, smem)) return rc;
+      k_mid_colp<R, TILE, +1><<<w->sm_count, 2 * R * TILE, smem, w->stream>>>(a);
+    }
+    return MMX_OK;
+  }
   if (dir < 0) {
     if (int rc = set_smem_col(k_mid_col<R, TILE, -1>, smem)) return rc;
     k_mid_col<R, TILE, -1><<<g, 2 * R * TILE, smem, w->stream>>>(a);

@@ -140,6 +140,7 @@ struct mmx_world {
   int nvec;            // S (+2 with elastic)
   size_t N;
   cudaStream_t stream;
+  int sm_count;        // multiprocessors of the device (grid size of the persistent kernels)
   int nreg;
   uint16_t* d_reg;
   std::vector<mmx_material> mats;  // [S][nreg]
@@ -225,6 +226,10 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L);
 bool mmx_mid_col_ok(int P, int n);
 int mmx_mid_col_launch(mmx_world* w, int P, int dir, const float2* in, float2* out, int n_in, int n_out,
                        size_t in_outer, size_t out_outer, int nslab, const float2* tw);
+
+// demag_x.cu: warp-per-row-pair x passes (fast path for Px = 512, one region)
+bool mmx_x_warp_ok(const mmx_world* w);
+int mmx_x_warp_launch(mmx_world* w, int dir, const float* const yin[2], float* bout);
 
 // local.cu
 int mmx_local_launch(mmx_world* w, const LocalArgs& a);
