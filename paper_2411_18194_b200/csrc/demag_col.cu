@@ -23,6 +23,9 @@ using namespace mmxreg;
 #ifndef MMX_MID_PERSISTENT
 #define MMX_MID_PERSISTENT 1
 #endif
+#ifndef MMX_INNER_VARIANT
+#define MMX_INNER_VARIANT 2   // 2: variant P (persistent, cp.async pipeline); 0: 32-column tiles (persistent when large), 1: variant W (16 columns, halves in one warp)
+#endif
 
 namespace {
 
@@ -169,6 +172,469 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_col(InnerColArgs a) {
       const int n = j + R * b;
       const float2 o = cadd(g[0][b], cmulc(g[1][b], stw[n]));
       if (ok && n < a.n_valid) base[(size_t)c * a.comp_stride + (size_t)n * a.line_stride] = o;
+    }
+  }
+}
+
+// Persistent form of k_inner_col: 2 CTAs per SM walk over the (ky, kx-tile) list; before a CTA
+// transforms a tile it asks L2 for the rows of its next tile (prefetch.global.L2: no registers,
+// no shared memory), so HBM keeps streaming while the SM computes and the loads of the next
+// iteration are L2 hits.  Tile order: ky and Py - ky are neighbours (same kernel rows).
+template <int R>
+__global__ void __launch_bounds__(32 * R, 2) k_inner_colp(InnerColArgs a) {
+  constexpr int H = R * R, P = 2 * H;
+  extern __shared__ float2 sm[];  // [6][H][32]
+  __shared__ float2 stw[P];
+  if (a.gated && !a.ctrl->active) return;
+  const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
+  for (int q = threadIdx.x; q < P; q += 32 * R) stw[q] = a.tw[q];
+  const int ntm = a.ntile_main * a.p_outer;
+  const int nt = ntm + (a.nyq ? (a.p_outer + 31) / 32 : 0);
+
+  auto locate = [&](int tile, int& kx, int& ko, bool& main_tile) -> bool {
+    bool ok;
+    main_tile = tile < ntm;
+    if (main_tile) {
+      const int yy = tile / a.ntile_main;
+      ko = (yy & 1) ? a.p_outer - ((yy + 1) >> 1) : (yy >> 1);
+      kx = (tile - yy * a.ntile_main) * 32 + lane; ok = kx < a.xc_main;
+    } else {
+      kx = a.xc - 1; ko = (tile - ntm) * 32 + lane; ok = ko < a.p_outer;
+    }
+    if (!ok) { kx = 0; ko = 0; }
+    return ok;
+  };
+  auto prefetch_tile = [&](int tile) {
+    if (tile >= ntm) return;  // Nyquist tiles are scattered and tiny
+    int kx, ko; bool mt;
+    locate(tile, kx, ko, mt);
+    const int kx0 = kx - lane;
+    const int kom = (2 * ko > a.p_outer) ? a.p_outer - ko : ko;
+    // spectrum rows: 3 components x n_valid rows x 256 B (two 128 B lines each)
+    for (int r = threadIdx.x; r < 3 * a.n_valid * 2; r += 32 * R) {
+      const int c = r / (2 * a.n_valid), rem = r - c * 2 * a.n_valid;
+      const int n = rem >> 1, hl = rem & 1;
+      prefetch_l2(a.spec + (size_t)ko * a.outer_stride + (size_t)c * a.comp_stride + (size_t)n * a.line_stride + kx0 + hl * 16);
+    }
+    for (int r = threadIdx.x; r < 6 * (H + 1); r += 32 * R) {
+      const int c = r / (H + 1), pm = r - c * (H + 1);
+      const float* p = a.khat + (size_t)kom * a.k_outer_stride + kx0 + (size_t)pm * a.k_inner_stride + (size_t)c * a.k_comp_stride;
+      prefetch_l2(p);
+      prefetch_l2(p + 31);
+    }
+  };
+
+  int tile = blockIdx.x;
+  if (tile < nt) prefetch_tile(tile);
+  __syncthreads();  // stw
+  for (; tile < nt; tile += gridDim.x) {
+    if (tile + (int)gridDim.x < nt) prefetch_tile(tile + gridDim.x);
+    int kx, ko; bool main_tile;
+    const bool ok = locate(tile, kx, ko, main_tile);
+    int kom = ko, so = 0;
+    if (a.p_outer > 1 && 2 * ko > a.p_outer) { kom = a.p_outer - ko; so = 1; }
+    const float* kb = a.khat + (size_t)kom * a.k_outer_stride + kx;
+    float2* base = a.spec + (size_t)ko * a.outer_stride + kx;
+    float2 x[3][R];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int u = 0; u < R; ++u) {
+        const int n = j + R * u;
+        x[c][u] = (ok && n < a.n_valid) ? base[(size_t)c * a.comp_stride + (size_t)n * a.line_stride]
+                                        : make_float2(0.f, 0.f);
+      }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        float2 v[R];
+#pragma unroll
+        for (int u = 0; u < R; ++u) v[u] = h ? cmul(x[c][u], stw[j + R * u]) : x[c][u];
+        Dft<R, -1>::run(v);
+        float2* t = sm + (size_t)(c * 2 + h) * H * 32 + lane;
+        t[(0 * R + j) * 32] = v[0];
+#pragma unroll
+        for (int q = 1; q < R; ++q) t[(q * R + j) * 32] = cmul(v[q], stw[2 * j * q]);
+      }
+    }
+    __syncthreads();
+    float2 X[3][2][R];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const float2* t = sm + (size_t)(c * 2 + h) * H * 32 + lane;
+#pragma unroll
+        for (int q = 0; q < R; ++q) X[c][h][q] = t[(j * R + q) * 32];
+        Dft<R, -1>::run(X[c][h]);
+      }
+    // sign masks of the odd components: xy is odd along the outer axis, xz along the inner one,
+    // yz along both (3-D); the 2-D caller passes its own odd_inner / odd_outer
+    const unsigned mo3 = (so & (a.odd_outer >> 3)) << 31, mo4 = (so & (a.odd_outer >> 4)) << 31, mo5 = (so & (a.odd_outer >> 5)) << 31;
+    const unsigned mi3 = ((a.odd_inner >> 3) & 1u) << 31, mi4 = ((a.odd_inner >> 4) & 1u) << 31, mi5 = ((a.odd_inner >> 5) & 1u) << 31;
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int b = 0; b < R; ++b) {
+        const int kz = 2 * (j + R * b) + h;
+        const bool mir = 2 * kz > P;
+        const int pm = mir ? P - kz : kz;
+        const float* kp = kb + (size_t)pm * a.k_inner_stride;
+        float K[6];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) K[c] = __ldg(kp + (size_t)c * a.k_comp_stride);
+        K[3] = __uint_as_float(__float_as_uint(K[3]) ^ mo3 ^ (mir ? mi3 : 0u));
+        K[4] = __uint_as_float(__float_as_uint(K[4]) ^ mo4 ^ (mir ? mi4 : 0u));
+        K[5] = __uint_as_float(__float_as_uint(K[5]) ^ mo5 ^ (mir ? mi5 : 0u));
+        const float2 mx = X[0][h][b], my = X[1][h][b], mz = X[2][h][b];
+        X[0][h][b] = make_float2(fmaf(K[0], mx.x, fmaf(K[3], my.x, K[4] * mz.x)),
+                                 fmaf(K[0], mx.y, fmaf(K[3], my.y, K[4] * mz.y)));
+        X[1][h][b] = make_float2(fmaf(K[3], mx.x, fmaf(K[1], my.x, K[5] * mz.x)),
+                                 fmaf(K[3], mx.y, fmaf(K[1], my.y, K[5] * mz.y)));
+        X[2][h][b] = make_float2(fmaf(K[4], mx.x, fmaf(K[5], my.x, K[2] * mz.x)),
+                                 fmaf(K[4], mx.y, fmaf(K[5], my.y, K[2] * mz.y)));
+      }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        Dft<R, +1>::run(X[c][h]);
+        float2* t = sm + (size_t)(c * 2 + h) * H * 32 + lane;
+        t[(j * R + 0) * 32] = X[c][h][0];
+#pragma unroll
+        for (int q = 1; q < R; ++q) t[(j * R + q) * 32] = cmulc(X[c][h][q], stw[2 * j * q]);
+      }
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      float2 g[2][R];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const float2* t = sm + (size_t)(c * 2 + h) * H * 32 + lane;
+#pragma unroll
+        for (int q = 0; q < R; ++q) g[h][q] = t[(q * R + j) * 32];
+        Dft<R, +1>::run(g[h]);
+      }
+#pragma unroll
+      for (int b = 0; b < R; ++b) {
+        const int n = j + R * b;
+        const float2 o = cadd(g[0][b], cmulc(g[1][b], stw[n]));
+        if (ok && n < a.n_valid) base[(size_t)c * a.comp_stride + (size_t)n * a.line_stride] = o;
+      }
+    }
+    __syncthreads();  // the exchange tiles are rewritten by the next iteration
+  }
+}
+
+// Variant W of the fused inner pass: 16 kx columns per CTA, lane = column + 16 h, so that the
+// two halves of a line sit in the same warp (their inputs are one load, their results meet by
+// shuffle) and a thread carries one half of three components (48 data registers): three CTAs
+// per SM instead of two.  The kernel-spectrum rows of the CTA (6 x (H+1) x 16 floats) are
+// copied to shared memory with cp.async at the start and waited for only before the multiply.
+__device__ __forceinline__ void cpa16(void* smem, const void* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+
+#ifndef MMX_INW_MINB
+#define MMX_INW_MINB 3
+#endif
+template <int R>
+__global__ void __launch_bounds__(32 * R, MMX_INW_MINB) k_inner_w(InnerColArgs a) {
+  constexpr int H = R * R, P = 2 * H, TL = 16;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  float2* sm = reinterpret_cast<float2*>(smraw);                          // [3][2][H][TL]
+  float* ks = reinterpret_cast<float*>(smraw + sizeof(float2) * 6 * H * TL);  // [6][H+1][TL]
+  __shared__ float2 stw[P];
+  if (a.gated && !a.ctrl->active) return;
+  const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
+  const int kxl = lane & 15, h = lane >> 4;
+  // blockIdx.y -> outer wave number: ky and p_outer - ky are neighbours in launch order (they
+  // read the same kernel rows, the second read hits L2)
+  int yy = blockIdx.y;
+  int kx, ko;
+  bool ok;
+  const bool main_tile = (int)blockIdx.x < a.ntile_main;
+  if (main_tile) {
+    ko = (yy & 1) ? a.p_outer - ((yy + 1) >> 1) : (yy >> 1);
+    kx = blockIdx.x * TL + kxl; ok = kx < a.xc_main;
+  } else {
+    if (yy * TL >= a.p_outer) return;
+    kx = a.xc - 1; ko = yy * TL + kxl; ok = ko < a.p_outer;
+  }
+  if (!ok) { kx = 0; ko = 0; }
+  for (int q = threadIdx.x; q < P; q += 32 * R) stw[q] = a.tw[q];
+  int kom = ko, so = 0;
+  if (a.p_outer > 1 && 2 * ko > a.p_outer) { kom = a.p_outer - ko; so = 1; }
+  if (main_tile) {
+    const float* kt = a.khat + (size_t)kom * a.k_outer_stride + (size_t)blockIdx.x * TL;
+    for (int r = threadIdx.x; r < 6 * (H + 1) * (TL / 4); r += 32 * R) {
+      const int row = r / (TL / 4), ch = r % (TL / 4);
+      const int c = row / (H + 1), pm = row % (H + 1);
+      cpa16(ks + (size_t)row * TL + 4 * ch, kt + (size_t)c * a.k_comp_stride + (size_t)pm * a.k_inner_stride + 4 * ch);
+    }
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+
+  float2* base = a.spec + (size_t)ko * a.outer_stride + kx;
+  float2 X[3][R];
+#pragma unroll
+  for (int c = 0; c < 3; ++c)
+#pragma unroll
+    for (int u = 0; u < R; ++u) {
+      const int n = j + R * u;
+      X[c][u] = (ok && n < a.n_valid) ? base[(size_t)c * a.comp_stride + (size_t)n * a.line_stride]
+                                      : make_float2(0.f, 0.f);
+    }
+  __syncthreads();  // stw
+  // forward stage 1 of this thread's half
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    if (h) {
+#pragma unroll
+      for (int u = 0; u < R; ++u) X[c][u] = cmul(X[c][u], stw[j + R * u]);
+    }
+    Dft<R, -1>::run(X[c]);
+    float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+    t[(0 * R + j) * TL] = X[c][0];
+#pragma unroll
+    for (int q = 1; q < R; ++q) t[(q * R + j) * TL] = cmul(X[c][q], stw[2 * j * q]);
+  }
+  __syncthreads();
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+#pragma unroll
+    for (int q = 0; q < R; ++q) X[c][q] = t[(j * R + q) * TL];
+    Dft<R, -1>::run(X[c]);
+  }
+  // B^_i = sum_j K^_ij M^_j ; K^ real, 6 unique components, octant + parity
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();  // kernel rows of all threads have landed
+  const float* kb = a.khat + (size_t)kom * a.k_outer_stride + kx;
+#pragma unroll
+  for (int b = 0; b < R; ++b) {
+    const int kz = 2 * (j + R * b) + h;
+    int pm = kz, si = 0;
+    if (2 * kz > P) { pm = P - kz; si = 1; }
+    float K[6];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      const float v = main_tile ? ks[((size_t)c * (H + 1) + pm) * TL + kxl]
+                                : __ldg(kb + (size_t)pm * a.k_inner_stride + (size_t)c * a.k_comp_stride);
+      const int flip = (si & (a.odd_inner >> c)) ^ (so & (a.odd_outer >> c));
+      K[c] = (flip & 1) ? -v : v;
+    }
+    const float2 mx = X[0][b], my = X[1][b], mz = X[2][b];
+    X[0][b] = make_float2(fmaf(K[0], mx.x, fmaf(K[3], my.x, K[4] * mz.x)),
+                          fmaf(K[0], mx.y, fmaf(K[3], my.y, K[4] * mz.y)));
+    X[1][b] = make_float2(fmaf(K[3], mx.x, fmaf(K[1], my.x, K[5] * mz.x)),
+                          fmaf(K[3], mx.y, fmaf(K[1], my.y, K[5] * mz.y)));
+    X[2][b] = make_float2(fmaf(K[4], mx.x, fmaf(K[5], my.x, K[2] * mz.x)),
+                          fmaf(K[4], mx.y, fmaf(K[5], my.y, K[2] * mz.y)));
+  }
+  // inverse stage 1 (over b); the thread writes the rows it has read: no barrier needed
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    Dft<R, +1>::run(X[c]);
+    float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+    t[(j * R + 0) * TL] = X[c][0];
+#pragma unroll
+    for (int q = 1; q < R; ++q) t[(j * R + q) * TL] = cmulc(X[c][q], stw[2 * j * q]);
+  }
+  __syncthreads();
+  // inverse stage 2, then x[n] = g0[n] + conj(w_P^n) g1[n]: lanes h = 0 finish rows b < R/2,
+  // lanes h = 1 rows b >= R/2, the other half's value arrives by shuffle
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+#pragma unroll
+    for (int q = 0; q < R; ++q) X[c][q] = t[(q * R + j) * TL];
+    Dft<R, +1>::run(X[c]);
+    if (h) {
+#pragma unroll
+      for (int b = 0; b < R; ++b) X[c][b] = cmulc(X[c][b], stw[j + R * b]);
+    }
+#pragma unroll
+    for (int bb = 0; bb < R / 2; ++bb) {
+      const float2 mine = h ? X[c][bb + R / 2] : X[c][bb];
+      const float2 send = h ? X[c][bb] : X[c][bb + R / 2];
+      float2 recv;
+      recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
+      recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+      const int n = j + R * (h ? bb + R / 2 : bb);
+      if (ok && n < a.n_valid)
+        base[(size_t)c * a.comp_stride + (size_t)n * a.line_stride] = cadd(mine, recv);
+    }
+  }
+}
+
+// Variant P of the fused inner pass: the thread mapping of variant W (16 columns, lane =
+// column + 16 h) in a persistent CTA with a two-stage cp.async pipeline.  While a CTA transforms
+// tile i out of one shared-memory stage, the rows of tile i+1 stream into the other, and the
+// kernel-spectrum values of tile i (48 per thread) are loaded into registers at the top of the
+// iteration, long before the multiply: no phase of the CTA waits for HBM.
+template <int BYTES>
+__device__ __forceinline__ void cpa_zfill(void* smem, const void* gmem, bool valid) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  const int n = valid ? BYTES : 0;
+  if (BYTES == 16)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(gmem), "r"(n) : "memory");
+  else
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(sa), "l"(gmem), "r"(n) : "memory");
+}
+
+template <int R>
+__global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
+  constexpr int H = R * R, P = 2 * H, TL = 16, NT = 32 * R;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  float2* sm = reinterpret_cast<float2*>(smraw);             // exchange [3][2][H][TL]
+  float2* stage = sm + (size_t)6 * H * TL;                   // input stages [2][3][H][TL]
+  __shared__ float2 stw[P];
+  if (a.gated && !a.ctrl->active) return;
+  const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
+  const int kxl = lane & 15, h = lane >> 4;
+  for (int q = threadIdx.x; q < P; q += NT) stw[q] = a.tw[q];
+  const int ntm = a.ntile_main * a.p_outer;
+  const int nt = ntm + (a.nyq ? (a.p_outer + TL - 1) / TL : 0);
+
+  // tile -> first column / outer index of lane l
+  auto tile_ko = [&](int tile) -> int {
+    const int yy = tile / a.ntile_main;
+    return (yy & 1) ? a.p_outer - ((yy + 1) >> 1) : (yy >> 1);
+  };
+  auto issue = [&](int tile, int buf) {
+    float2* dst = stage + (size_t)buf * 3 * H * TL;
+    if (tile < ntm) {
+      const int yy = tile / a.ntile_main;
+      const int ko = (yy & 1) ? a.p_outer - ((yy + 1) >> 1) : (yy >> 1);
+      const int kx0 = (tile - yy * a.ntile_main) * TL;
+      const float2* src = a.spec + (size_t)ko * a.outer_stride + kx0;
+      // 3 H rows of TL float2 = 8 chunks of 16 B each
+      for (int q = threadIdx.x; q < 3 * H * (TL / 2); q += NT) {
+        const int row = q / (TL / 2), ch = q % (TL / 2);
+        const int c = row / H, n = row % H;
+        cpa_zfill<16>(dst + (size_t)row * TL + 2 * ch,
+                      src + (size_t)c * a.comp_stride + (size_t)n * a.line_stride + 2 * ch, n < a.n_valid);
+      }
+    } else {
+      const int ko0 = (tile - ntm) * TL;
+      for (int q = threadIdx.x; q < 3 * H * TL; q += NT) {
+        const int row = q / TL, l = q % TL;
+        const int c = row / H, n = row % H;
+        const bool v = n < a.n_valid && ko0 + l < a.p_outer;
+        const int ko = v ? ko0 + l : 0;
+        cpa_zfill<8>(dst + (size_t)row * TL + l,
+                     a.spec + (size_t)ko * a.outer_stride + (a.xc - 1) + (size_t)c * a.comp_stride + (size_t)n * a.line_stride, v);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  int tile = blockIdx.x;
+  if (tile < nt) issue(tile, 0);
+  int buf = 0;
+  for (; tile < nt; tile += gridDim.x, buf ^= 1) {
+    const int nxt = tile + gridDim.x;
+    if (nxt < nt) issue(nxt, buf ^ 1);
+    // where this thread's column lives
+    int kx, ko;
+    bool ok = true;
+    const bool main_tile = tile < ntm;
+    if (main_tile) {
+      ko = tile_ko(tile);
+      kx = (tile - (tile / a.ntile_main) * a.ntile_main) * TL + kxl;
+      ok = kx < a.xc_main;  // (columns up to the row pitch exist: reads are safe, stores are masked)
+    } else {
+      kx = a.xc - 1; ko = (tile - ntm) * TL + kxl; ok = ko < a.p_outer;
+      if (!ok) ko = 0;
+    }
+    int kom = ko, so = 0;
+    if (a.p_outer > 1 && 2 * ko > a.p_outer) { kom = a.p_outer - ko; so = 1; }
+    // kernel spectrum of this thread's 8 wave numbers: issued now, used after the forward transform
+    const float* kb = a.khat + (size_t)kom * a.k_outer_stride + kx;
+    float K[R][6];
+#pragma unroll
+    for (int b = 0; b < R; ++b) {
+      const int kz = 2 * (j + R * b) + h;
+      const int pm = 2 * kz > P ? P - kz : kz;
+#pragma unroll
+      for (int c = 0; c < 6; ++c) K[b][c] = __ldg(kb + (size_t)pm * a.k_inner_stride + (size_t)c * a.k_comp_stride);
+    }
+    if (nxt < nt) asm volatile("cp.async.wait_group 1;" ::: "memory");
+    else asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();  // tile i has landed for every thread; exchange tiles of tile i-1 are free
+    const float2* xin = stage + (size_t)buf * 3 * H * TL + kxl;
+    float2 X[3][R];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+      for (int u = 0; u < R; ++u) X[c][u] = xin[(size_t)(c * H + j + R * u) * TL];
+      if (h) {
+#pragma unroll
+        for (int u = 0; u < R; ++u) X[c][u] = cmul(X[c][u], stw[j + R * u]);
+      }
+      Dft<R, -1>::run(X[c]);
+      float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+      t[(0 * R + j) * TL] = X[c][0];
+#pragma unroll
+      for (int q = 1; q < R; ++q) t[(q * R + j) * TL] = cmul(X[c][q], stw[2 * j * q]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+#pragma unroll
+      for (int q = 0; q < R; ++q) X[c][q] = t[(j * R + q) * TL];
+      Dft<R, -1>::run(X[c]);
+    }
+    // B^_i = sum_j K^_ij M^_j ; K^ real, octant + parity (sign bit flips)
+    const unsigned mo3 = (so & (a.odd_outer >> 3)) << 31, mo4 = (so & (a.odd_outer >> 4)) << 31, mo5 = (so & (a.odd_outer >> 5)) << 31;
+    const unsigned mi3 = ((a.odd_inner >> 3) & 1u) << 31, mi4 = ((a.odd_inner >> 4) & 1u) << 31, mi5 = ((a.odd_inner >> 5) & 1u) << 31;
+#pragma unroll
+    for (int b = 0; b < R; ++b) {
+      const bool mir = 2 * (2 * (j + R * b) + h) > P;
+      const float k0 = K[b][0], k1 = K[b][1], k2 = K[b][2];
+      const float k3 = __uint_as_float(__float_as_uint(K[b][3]) ^ mo3 ^ (mir ? mi3 : 0u));
+      const float k4 = __uint_as_float(__float_as_uint(K[b][4]) ^ mo4 ^ (mir ? mi4 : 0u));
+      const float k5 = __uint_as_float(__float_as_uint(K[b][5]) ^ mo5 ^ (mir ? mi5 : 0u));
+      const float2 mx = X[0][b], my = X[1][b], mz = X[2][b];
+      X[0][b] = make_float2(fmaf(k0, mx.x, fmaf(k3, my.x, k4 * mz.x)), fmaf(k0, mx.y, fmaf(k3, my.y, k4 * mz.y)));
+      X[1][b] = make_float2(fmaf(k3, mx.x, fmaf(k1, my.x, k5 * mz.x)), fmaf(k3, mx.y, fmaf(k1, my.y, k5 * mz.y)));
+      X[2][b] = make_float2(fmaf(k4, mx.x, fmaf(k5, my.x, k2 * mz.x)), fmaf(k4, mx.y, fmaf(k5, my.y, k2 * mz.y)));
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      Dft<R, +1>::run(X[c]);
+      float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+      t[(j * R + 0) * TL] = X[c][0];
+#pragma unroll
+      for (int q = 1; q < R; ++q) t[(j * R + q) * TL] = cmulc(X[c][q], stw[2 * j * q]);
+    }
+    __syncthreads();
+    float2* base = a.spec + (size_t)ko * a.outer_stride + kx;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+#pragma unroll
+      for (int q = 0; q < R; ++q) X[c][q] = t[(q * R + j) * TL];
+      Dft<R, +1>::run(X[c]);
+      if (h) {
+#pragma unroll
+        for (int b = 0; b < R; ++b) X[c][b] = cmulc(X[c][b], stw[j + R * b]);
+      }
+#pragma unroll
+      for (int bb = 0; bb < R / 2; ++bb) {
+        const float2 mine = h ? X[c][bb + R / 2] : X[c][bb];
+        const float2 send = h ? X[c][bb] : X[c][bb + R / 2];
+        float2 recv;
+        recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
+        recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+        const int n = j + R * (h ? bb + R / 2 : bb);
+        if (ok && n < a.n_valid)
+          base[(size_t)c * a.comp_stride + (size_t)n * a.line_stride] = cadd(mine, recv);
+      }
     }
   }
 }
@@ -373,7 +839,8 @@ __global__ void __launch_bounds__(2 * R * TILE, 1) k_mid_colp(MidColArgs a) {
 
 template <typename Kern>
 int set_smem_col(Kern k, size_t bytes) {
-  if (bytes > 48 * 1024) MMX_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  // (the kernels also hold a static twiddle table: the 48 KB default limit counts both)
+  if (bytes > 32 * 1024) MMX_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
   return MMX_OK;
 }
 
@@ -391,17 +858,44 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   InnerColArgs a;
   a.spec = L.spec; a.khat = d.khat; a.tw = L.tw; a.ctrl = w->d_ctrl; a.gated = 1;
   a.n_valid = L.n_valid; a.xc = d.xc; a.p_outer = L.p_outer;
-  a.nyq = ((d.xc - 1) % 32 == 0 && d.xc > 1 && L.n_outer >= 32) ? 1 : 0;
-  if (a.nyq) { a.ntile_main = (d.xc - 1) / 32; a.xc_main = d.xc - 1; }
-  else { a.ntile_main = (d.xc + 31) / 32; a.xc_main = d.xc; }
+#if MMX_INNER_VARIANT >= 1
+  constexpr int TL = 16;
+#else
+  constexpr int TL = 32;
+#endif
+  a.nyq = ((d.xc - 1) % TL == 0 && d.xc > 1 && L.n_outer >= TL && L.p_outer == L.n_outer) ? 1 : 0;
+  if (a.nyq) { a.ntile_main = (d.xc - 1) / TL; a.xc_main = d.xc - 1; }
+  else { a.ntile_main = (d.xc + TL - 1) / TL; a.xc_main = d.xc; }
   a.line_stride = L.line_stride; a.comp_stride = L.comp_stride; a.outer_stride = L.outer_stride;
   a.k_inner_stride = L.k_inner_stride; a.k_outer_stride = L.k_outer_stride; a.k_comp_stride = L.k_comp_stride;
   a.odd_inner = L.odd_inner; a.odd_outer = L.odd_outer;
-  const size_t smem = sizeof(float2) * 6 * 64 * 32;
-  if (int rc = set_smem_col(k_inner_col<8>, smem)) return rc;
-  dim3 g(a.ntile_main + a.nyq, L.n_outer);
   ProfScope ps(w, PK_INNER);
-  k_inner_col<8><<<g, 256, smem, w->stream>>>(a);
+#if MMX_INNER_VARIANT == 2
+  const size_t smem = sizeof(float2) * (6 + 6) * 64 * TL;
+  if (int rc = set_smem_col(k_inner_pipe<8>, smem)) return rc;
+  const int nt = a.ntile_main * L.n_outer + (a.nyq ? (L.p_outer + TL - 1) / TL : 0);
+  int grid = 2 * w->sm_count;
+  if (grid > nt) grid = nt;
+  if (L.p_outer != L.n_outer) return mmx_fail(MMX_EINVAL, "inner column pass: outer extent mismatch");
+  k_inner_pipe<8><<<grid, 256, smem, w->stream>>>(a);
+#elif MMX_INNER_VARIANT == 1
+  const size_t smem = sizeof(float2) * 6 * 64 * TL + sizeof(float) * 6 * 65 * TL;
+  if (int rc = set_smem_col(k_inner_w<8>, smem)) return rc;
+  dim3 g(a.ntile_main + a.nyq, L.n_outer);
+  k_inner_w<8><<<g, 256, smem, w->stream>>>(a);
+#else
+  const size_t smem = sizeof(float2) * 6 * 64 * TL;
+  const int nt = a.ntile_main * L.n_outer + (a.nyq ? (L.p_outer + 31) / 32 : 0);
+  if (L.p_outer == L.n_outer && nt >= 8 * w->sm_count) {
+    if (int rc = set_smem_col(k_inner_colp<8>, smem)) return rc;
+    k_inner_colp<8><<<2 * w->sm_count, 256, smem, w->stream>>>(a);
+  } else {
+    if (int rc = set_smem_col(k_inner_col<8>, smem)) return rc;
+    dim3 g(a.ntile_main + a.nyq, L.n_outer);
+    k_inner_col<8><<<g, 256, smem, w->stream>>>(a);
+  }
+#endif
+  MMX_CUDA(cudaGetLastError());
   return MMX_OK;
 }
 
@@ -424,6 +918,7 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
       if (int rc = set_smem_col(k_mid_colp<R, TILE, +1>, smem)) return rc;
       k_mid_colp<R, TILE, +1><<<w->sm_count, 2 * R * TILE, smem, w->stream>>>(a);
     }
+    MMX_CUDA(cudaGetLastError());
     return MMX_OK;
   }
   if (dir < 0) {
@@ -433,6 +928,7 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
     if (int rc = set_smem_col(k_mid_col<R, TILE, +1>, smem)) return rc;
     k_mid_col<R, TILE, +1><<<g, 2 * R * TILE, smem, w->stream>>>(a);
   }
+  MMX_CUDA(cudaGetLastError());
   return MMX_OK;
 }
 

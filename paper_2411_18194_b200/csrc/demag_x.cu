@@ -244,5 +244,6 @@ int mmx_x_warp_launch(mmx_world* w, int dir, const float* const yin[2], float* b
     ProfScope ps(w, PK_X_INV);
     k_x_inv_w<<<blocks, 32 * XW, smem, w->stream>>>(a);
   }
+  MMX_CUDA(cudaGetLastError());
   return MMX_OK;
 }

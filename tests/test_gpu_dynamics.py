@@ -1,5 +1,5 @@
-"""GPU parity, dynamics: fixed-step trajectories of every config (reduced sizes here, the
-BASELINE.json sizes in test_gpu_fullsize.py) against the fp64 oracle: max |delta m| <= 1e-4
+"""GPU parity, dynamics: fixed-step trajectories of every config (reduced sizes here; the full-size c4 field check is in
+test_gpu_fields.py) against the fp64 oracle: max |delta m| <= 1e-4
 (north_star), DP45 error estimates, the adaptive controller, |m| = 1."""
 import numpy as np
 import pytest
@@ -31,6 +31,7 @@ def test_c1_rk4_full_protocol():
 
 @pytest.mark.parametrize("name,grid,nsteps", [("c2", (64, 64, 1), 200), ("c3", (128, 32, 1), 200),
                                               ("c4", (32, 32, 8), 100), ("c4", (20, 12, 3), 50),
+                                              ("c4", (136, 40, 36), 30),  # register-resident fast paths
                                               ("c5", (64, 32, 1), 200)])
 def test_dp45_fixed_step_trajectory(name, grid, nsteps):
     spec = wl.make(name, grid)

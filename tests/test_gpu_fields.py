@@ -169,3 +169,61 @@ def test_elastic_3d_and_periodic():
     for s in range(2):
         assert field_err(g.eval_heff(s, mmx.T_MEL), o.field_terms(s, terms=oc.T_MEL)[oc.T_MEL]) < FIELD_TOL
     g.destroy()
+
+
+# ---- the register-resident fast paths (Px = 512 warp x passes, column y / z passes, float4 local
+# kernel) only engage on grids shaped like c4; these cases are the smallest ones that reach every
+# variant: mid pass R = 4 (Py = 32), R = 8 (Py = 128), R = 16 (Py = 512), inner pass P = 128.
+FAST_CASES = [(132, 12, 40), (136, 40, 36), (256, 130, 33), (192, 64, 64)]
+
+
+@pytest.mark.parametrize("grid", FAST_CASES)
+def test_fast_path_fields(grid):
+    spec = _rich_spec("c4", grid, seed=11)
+    g, o = pair(spec)
+    ref = o.field_terms(0)
+    for tname in ("demag", "exch", "dmi", "anis_u", "anis_c", "zeeman"):
+        bit = TERMS[tname]
+        e = field_err(g.eval_heff(0, bit), ref[bit])
+        assert e < FIELD_TOL, (grid, tname, e)
+    e = field_err(g.eval_heff(0, mmx.T_ALL), o.heff(0))
+    assert e < FIELD_TOL, (grid, "total", e)
+    e = field_err(g.eval_torque(0), o.torque(0))
+    assert e < FIELD_TOL, (grid, "torque", e)
+    g.destroy()
+
+
+def test_fast_path_two_sublattices():
+    """S = 2, one region: the x pass forms M = Ms1 m1 + Ms2 m2 while reading."""
+    spec = _rich_spec("c3", (132, 12, 40), seed=5)
+    spec.regions = None
+    for k, v in spec.mat.items():
+        spec.mat[k] = v[:, :1].copy()
+    spec.mat["Ms"][1] *= 0.7
+    g, o = pair(spec)
+    for s in range(2):
+        e = field_err(g.eval_heff(s, mmx.T_ALL), o.heff(s))
+        assert e < FIELD_TOL, (s, e)
+    g.destroy()
+
+
+def test_c4_full_size_sampled_against_direct_sum():
+    """BASELINE config 4 at full size (256x256x64, the launch configuration bench.py times): the
+    demag field at sampled cells against the oracle's O(N) direct sum per cell (the definition),
+    and the exchange field against the oracle on the whole grid."""
+    spec = wl.make("c4")
+    assert tuple(spec.grid) == (256, 256, 64)
+    g, o = pair(spec)
+    B = g.eval_heff(0, mmx.T_DEMAG).astype(np.float64)
+    rng = np.random.default_rng(123)
+    targets = [(0, 0, 0), (255, 255, 63), (255, 0, 63), (128, 128, 32), (1, 254, 31)]
+    targets += [tuple(int(v) for v in (rng.integers(256), rng.integers(256), rng.integers(64))) for _ in range(7)]
+    ref = o.demag_field(o.m, targets=targets)
+    rms = np.sqrt((B ** 2).sum(axis=0).mean())
+    for t, (ix, iy, iz) in enumerate(targets):
+        d = np.linalg.norm(B[:, iz, iy, ix] - ref[:, t])
+        n = max(np.linalg.norm(ref[:, t]), 0.1 * rms)
+        assert d / n < FIELD_TOL, ((ix, iy, iz), d / n)
+    e = field_err(g.eval_heff(0, mmx.T_EXCH), o.field_terms(0, terms=oc.T_EXCH)[oc.T_EXCH])
+    assert e < FIELD_TOL, e
+    g.destroy()
