@@ -910,7 +910,9 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
   const size_t smem = sizeof(float2) * (dir < 0 ? 2 : 3) * R * R * TILE;
   ProfScope ps(w, dir < 0 ? PK_MID_FWD : PK_MID_INV);
   const int ntiles = a.ntile_main * a.nslab + (a.nyq ? (a.nslab + TILE - 1) / TILE : 0);
-  if (MMX_MID_PERSISTENT && ntiles >= 4 * w->sm_count) {
+  // measured on c4: the register-prefetching persistent form wins for the inverse pass (89 vs 95 us),
+  // the plain grid for the forward pass (80 vs 90 us)
+  if (MMX_MID_PERSISTENT && dir > 0 && ntiles >= 4 * w->sm_count) {
     if (dir < 0) {
       if (int rc = set_smem_col(k_mid_colp<R, TILE, -1>, smem)) return rc;
       k_mid_colp<R, TILE, -1><<<w->sm_count, 2 * R * TILE, smem, w->stream>>>(a);

@@ -273,11 +273,30 @@ __device__ __forceinline__ void stq(float* p, size_t N, size_t i, const Q3& q) {
 // state, bit 1: form the embedded error
 template <int S, int NP, int MODE>
 __global__ void __launch_bounds__(256, MMX_L4_MINB) k_local4(LocalArgs a) {
+  // thread-private landing slots for the streamed inputs (B_demag, y0, k_j): cp.async puts them
+  // in flight at the top of the kernel without holding registers; slot a of thread t is
+  // lsm[a * 256 + t] (16 B per lane: conflict-free)
+  extern __shared__ float4 lsm[];
   MmxCtrl* ctrl = a.ctrl;
   if (!ctrl->active) return;
   const int sel = ctrl->sel;
   const size_t N = (size_t)a.nx * a.ny * a.nz;
   const unsigned gpr = a.nx >> 2;  // groups per row
+  auto stage3 = [&](int slot, const float* p, size_t idx) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const unsigned sa = (unsigned)__cvta_generic_to_shared(&lsm[(slot + c) * 256 + threadIdx.x]);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(p + (size_t)c * N + idx) : "memory");
+    }
+  };
+  auto take3 = [&](int slot) -> Q3 {
+    const float4 x = lsm[(slot + 0) * 256 + threadIdx.x];
+    const float4 y = lsm[(slot + 1) * 256 + threadIdx.x];
+    const float4 z = lsm[(slot + 2) * 256 + threadIdx.x];
+    Q3 q;
+    q.c[0] = v3(x.x, y.x, z.x); q.c[1] = v3(x.y, y.y, z.y); q.c[2] = v3(x.z, y.z, z.z); q.c[3] = v3(x.w, y.w, z.w);
+    return q;
+  };
   const unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   const unsigned rows = (unsigned)a.ny * a.nz;
   const float* yin = a.yin[sel];
@@ -313,32 +332,23 @@ __global__ void __launch_bounds__(256, MMX_L4_MINB) k_local4(LocalArgs a) {
         if (s != a.heff_s) continue;
       }
       const int o = S == 2 ? 1 - s : s;
-      // RK epilogue inputs first (independent of the field): ys = y0 + sum_j ca_j k_j, er = sum_j ce_j k_j
+      // streamed inputs of this sublattice: slot 0 B_demag, slot 3 y0, slot 6 + 3 j k_j
       constexpr bool comb = (MODE & 1) != 0, doerr = (MODE & 2) != 0;
       const bool epi = !a.heff_out && !a.tau_out;
       const float* ca = ctrl->ca[a.combine_row];
       const float* ce = ctrl->ce;
-      Q3 ys, er;
+      const bool use_bd = (a.terms & MMX_T_DEMAG) && a.bdemag;
+      if (use_bd) stage3(0, a.bdemag, i);
       if (MODE != 0 && epi) {
-        if (comb) ys = ldq(a.y0[sel] + (size_t)s * 3 * N, N, i);
-        if (doerr) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) er.c[e] = v3(0.f, 0.f, 0.f);
-        }
+        if (comb) stage3(3, a.y0[sel] + (size_t)s * 3 * N, i);
 #pragma unroll
         for (int j = 0; j < NP; ++j) {
           const float cj = comb ? ca[j] : 0.f;
           const float ej = doerr ? ce[j] : 0.f;
-          if (cj != 0.f || ej != 0.f) {
-            const Q3 kj = ldq(a.kprev[sel][j] + (size_t)s * 3 * N, N, i);
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              if (comb) ys.c[e] = fma3(cj, kj.c[e], ys.c[e]);
-              if (doerr) er.c[e] = fma3(ej, kj.c[e], er.c[e]);
-            }
-          }
+          if (cj != 0.f || ej != 0.f) stage3(6 + 3 * j, a.kprev[sel][j] + (size_t)s * 3 * N, i);
         }
       }
+      asm volatile("cp.async.commit_group;" ::: "memory");
       const float* P = a.mat + (size_t)s * MMX_MATW;
       const float iMs = P[MP_INVMS];
       const float* ms_ = yin + (size_t)s * 3 * N;
@@ -402,8 +412,8 @@ __global__ void __launch_bounds__(256, MMX_L4_MINB) k_local4(LocalArgs a) {
         }
       }
       Q3 bd, tau;
-      const bool use_bd = (a.terms & MMX_T_DEMAG) && a.bdemag;
-      if (use_bd) bd = ldq(a.bdemag, N, i);
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      if (use_bd) bd = take3(0);
       float eps[6][4];
       const bool use_mel = (a.terms & MMX_T_MEL) && a.strain;
       if (use_mel) {
@@ -463,6 +473,27 @@ __global__ void __launch_bounds__(256, MMX_L4_MINB) k_local4(LocalArgs a) {
           const float t2 = dot(tau.c[e], tau.c[e]);
           tqv = fmaxf(tqv, sqrtf(t2));
           bad |= !(t2 == t2);
+        }
+      }
+      Q3 ys, er;
+      if (MODE != 0 && epi) {
+        if (comb) ys = take3(3);
+        if (doerr) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) er.c[e] = v3(0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int j = 0; j < NP; ++j) {
+          const float cj = comb ? ca[j] : 0.f;
+          const float ej = doerr ? ce[j] : 0.f;
+          if (cj != 0.f || ej != 0.f) {
+            const Q3 kj = take3(6 + 3 * j);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              if (comb) ys.c[e] = fma3(cj, kj.c[e], ys.c[e]);
+              if (doerr) er.c[e] = fma3(ej, kj.c[e], er.c[e]);
+            }
+          }
         }
       }
       if (comb) {
@@ -613,12 +644,19 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   if (uniform) {
     const unsigned b4 = (unsigned)((N / 4 + 255) / 256);
     const int mode = (a.ynext[0] ? 1 : 0) | (a.do_err ? 2 : 0);
+#define MMX_L4_GO(S_, NP_, M_)                                                             \
+  {                                                                                        \
+    const size_t sm_ = sizeof(float4) * 256 * (6 + 3 * (NP_));                             \
+    if (sm_ > 32 * 1024)                                                                   \
+      MMX_CUDA(cudaFuncSetAttribute(k_local4<S_, NP_, M_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_)); \
+    k_local4<S_, NP_, M_><<<b4, 256, sm_, w->stream>>>(a);                                 \
+  }
 #define MMX_L4(S_, NP_)                                                    \
   case NP_:                                                                \
-    if (mode == 0) k_local4<S_, 0, 0><<<b4, 256, 0, w->stream>>>(a);       \
-    else if (mode == 1) k_local4<S_, NP_, 1><<<b4, 256, 0, w->stream>>>(a); \
-    else if (mode == 2) k_local4<S_, NP_, 2><<<b4, 256, 0, w->stream>>>(a); \
-    else k_local4<S_, NP_, 3><<<b4, 256, 0, w->stream>>>(a);               \
+    if (mode == 0) MMX_L4_GO(S_, 0, 0)                                     \
+    else if (mode == 1) MMX_L4_GO(S_, NP_, 1)                              \
+    else if (mode == 2) MMX_L4_GO(S_, NP_, 2)                              \
+    else MMX_L4_GO(S_, NP_, 3)                                             \
     break;
 #define MMX_L4_ALL(S_) switch (a.n_prev) { MMX_L4(S_, 0) MMX_L4(S_, 1) MMX_L4(S_, 2) MMX_L4(S_, 3) MMX_L4(S_, 4) \
     MMX_L4(S_, 5) MMX_L4(S_, 6) MMX_L4(S_, 7) default: return mmx_fail(MMX_EINVAL, "n_prev %d out of range", a.n_prev); }
