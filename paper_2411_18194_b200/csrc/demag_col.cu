@@ -23,6 +23,9 @@ using namespace mmxreg;
 #ifndef MMX_MID_PERSISTENT
 #define MMX_MID_PERSISTENT 1
 #endif
+#ifndef MMX_MID_PIPE
+#define MMX_MID_PIPE 1        // 1: pipelined y pass (cp.async stages) for 512-point lines on large grids
+#endif
 #ifndef MMX_INNER_VARIANT
 #define MMX_INNER_VARIANT 2   // 2: variant P (persistent, cp.async pipeline); 0: 32-column tiles (persistent when large), 1: variant W (16 columns, halves in one warp)
 #endif
@@ -837,6 +840,127 @@ __global__ void __launch_bounds__(2 * R * TILE, 1) k_mid_colp(MidColArgs a) {
   }
 }
 
+// Pipelined y pass (P = 2 R^2): persistent CTAs of 8 columns x R threads per line x 2 halves
+// (lane = column + 8 h + 16 (j & 1)), the rows of the next tile stream into shared memory with
+// cp.async while the current tile is transformed; the halves of the inverse meet by shuffle.
+// Small CTAs (16 R threads, 65-97 KB) so that three (forward) or two (inverse) of them share an SM.
+#ifndef MMX_MIDP_MINB_F
+#define MMX_MIDP_MINB_F 3
+#endif
+#ifndef MMX_MIDP_MINB_I
+#define MMX_MIDP_MINB_I 2
+#endif
+template <int R, int DIR>
+__global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_MINB_I) k_mid_pipe(MidColArgs a) {
+  constexpr int H = R * R, P = 2 * H, TL = 8, NT = 16 * R;
+  constexpr int ROWS = DIR < 0 ? H : P;   // rows of a staged tile
+  constexpr int EXT = H * TL + 8;         // exchange tile of one half (+8: the halves use different banks)
+  extern __shared__ __align__(16) unsigned char smraw[];
+  float2* exb = reinterpret_cast<float2*>(smraw);   // [2][EXT]
+  float2* stage = exb + 2 * EXT;                     // [2][ROWS][TL]
+  __shared__ float2 stw[P];
+  if (a.gated && !a.ctrl->active) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int kxl = lane & 7, h = (lane >> 3) & 1, j = 2 * wid + (lane >> 4);
+  for (int q = threadIdx.x; q < P; q += NT) stw[q] = a.tw[q];
+  const int ntm = a.ntile_main * a.nslab;
+  const int nt = ntm + (a.nyq ? (a.nslab + TL - 1) / TL : 0);
+  float2* ex = exb + h * EXT + kxl;
+
+  auto issue = [&](int tile, int buf) {
+    float2* dst = stage + (size_t)buf * ROWS * TL;
+    if (tile < ntm) {
+      const int slab = tile / a.ntile_main;
+      const int kx0 = (tile - slab * a.ntile_main) * TL;
+      const float2* src = a.in + (size_t)slab * a.in_outer + kx0;
+#pragma unroll
+      for (int q0 = 0; q0 < ROWS * (TL / 2); q0 += NT) {
+        const int q = q0 + threadIdx.x;
+        const int row = q / (TL / 2), ch = q % (TL / 2);
+        cpa_zfill<16>(dst + row * TL + 2 * ch, src + (size_t)row * a.xp + 2 * ch, row < a.n_in);
+      }
+    } else {
+      const int slab0 = (tile - ntm) * TL;
+      for (int q = threadIdx.x; q < ROWS * TL; q += NT) {
+        const int row = q / TL, l = q % TL;
+        const bool v = row < a.n_in && slab0 + l < a.nslab;
+        const int slab = v ? slab0 + l : 0;
+        cpa_zfill<8>(dst + row * TL + l, a.in + (size_t)slab * a.in_outer + (size_t)row * a.xp + (a.xc - 1), v);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  int tile = blockIdx.x;
+  if (tile < nt) issue(tile, 0);
+  int buf = 0;
+  for (; tile < nt; tile += gridDim.x, buf ^= 1) {
+    const int nxt = tile + gridDim.x;
+    if (nxt < nt) {
+      issue(nxt, buf ^ 1);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();  // tile landed for all threads; exchange tiles of the previous tile are free
+    int kx, slab;
+    bool ok = true;
+    if (tile < ntm) {
+      slab = tile / a.ntile_main;
+      kx = (tile - slab * a.ntile_main) * TL + kxl;
+      ok = kx < a.xc_main;
+    } else {
+      kx = a.xc - 1; slab = (tile - ntm) * TL + kxl; ok = slab < a.nslab;
+      if (!ok) slab = 0;
+    }
+    const float2* xin = stage + (size_t)buf * ROWS * TL + kxl;
+    float2 v[R];
+    if (DIR < 0) {
+#pragma unroll
+      for (int u = 0; u < R; ++u) {
+        const float2 x = xin[(j + R * u) * TL];
+        const float2 w = h ? stw[j + R * u] : make_float2(1.f, 0.f);
+        v[u] = cmul(x, w);
+      }
+    } else {
+#pragma unroll
+      for (int u = 0; u < R; ++u) v[u] = xin[(2 * (j + R * u) + h) * TL];
+    }
+    Dft<R, DIR>::run(v);
+    ex[(0 * R + j) * TL] = v[0];
+#pragma unroll
+    for (int q = 1; q < R; ++q) ex[(q * R + j) * TL] = ctw<DIR>(v[q], stw[2 * j * q]);
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < R; ++q) v[q] = ex[(j * R + q) * TL];
+    Dft<R, DIR>::run(v);
+    float2* out = a.out + (size_t)slab * a.out_outer + kx;
+    if (DIR < 0) {
+      if (ok) {
+#pragma unroll
+        for (int b = 0; b < R; ++b) out[(size_t)(2 * (j + R * b) + h) * a.xp] = v[b];
+      }
+    } else {
+      // x[n] = g0[n] + conj(w_P^n) g1[n]: lanes h = 0 finish rows b < R/2, lanes h = 1 the others
+#pragma unroll
+      for (int b = 0; b < R; ++b) {
+        const float2 w = h ? stw[j + R * b] : make_float2(1.f, 0.f);
+        v[b] = cmulc(v[b], w);
+      }
+#pragma unroll
+      for (int bb = 0; bb < R / 2; ++bb) {
+        const float2 mine = h ? v[bb + R / 2] : v[bb];
+        const float2 send = h ? v[bb] : v[bb + R / 2];
+        float2 recv;
+        recv.x = __shfl_xor_sync(0xffffffffu, send.x, 8);
+        recv.y = __shfl_xor_sync(0xffffffffu, send.y, 8);
+        const int n = j + R * (h ? bb + R / 2 : bb);
+        if (ok && n < a.n_out) out[(size_t)n * a.xp] = cadd(mine, recv);
+      }
+    }
+  }
+}
+
 template <typename Kern>
 int set_smem_col(Kern k, size_t bytes) {
   // (the kernels also hold a static twiddle table: the 48 KB default limit counts both)
@@ -912,6 +1036,28 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
   const int ntiles = a.ntile_main * a.nslab + (a.nyq ? (a.nslab + TILE - 1) / TILE : 0);
   // measured on c4: the register-prefetching persistent form wins for the inverse pass (89 vs 95 us),
   // the plain grid for the forward pass (80 vs 90 us)
+#if MMX_MID_PIPE
+  if (R == 16 && ntiles >= 8 * w->sm_count) {
+    MidColArgs b = a;
+    constexpr int TL = 8;
+    b.nyq = ((a.xc - 1) % TL == 0 && a.xc > 1 && a.nslab >= TL) ? 1 : 0;
+    if (b.nyq) { b.ntile_main = (a.xc - 1) / TL; b.xc_main = a.xc - 1; }
+    else { b.ntile_main = (a.xc + TL - 1) / TL; b.xc_main = a.xc; }
+    const int nt = b.ntile_main * a.nslab + (b.nyq ? (a.nslab + TL - 1) / TL : 0);
+    const size_t sm = sizeof(float2) * (2 * (R * R * TL + 8) + 2 * (dir < 0 ? R * R : 2 * R * R) * TL);
+    if (dir < 0) {
+      if (int rc = set_smem_col(k_mid_pipe<16, -1>, sm)) return rc;
+      int grid = MMX_MIDP_MINB_F * w->sm_count;
+      k_mid_pipe<16, -1><<<grid < nt ? grid : nt, 16 * 16, sm, w->stream>>>(b);
+    } else {
+      if (int rc = set_smem_col(k_mid_pipe<16, +1>, sm)) return rc;
+      int grid = MMX_MIDP_MINB_I * w->sm_count;
+      k_mid_pipe<16, +1><<<grid < nt ? grid : nt, 16 * 16, sm, w->stream>>>(b);
+    }
+    MMX_CUDA(cudaGetLastError());
+    return MMX_OK;
+  }
+#endif
   if (MMX_MID_PERSISTENT && dir > 0 && ntiles >= 4 * w->sm_count) {
     if (dir < 0) {
       if (int rc = set_smem_col(k_mid_colp<R, TILE, -1>, smem)) return rc;

@@ -22,7 +22,8 @@ namespace {
 
 constexpr int XR = 16, XH = 256, XP = 512;
 constexpr int XW = 8;                 // warps per CTA
-constexpr int EXN = XH + XH / 16;     // padded exchange tile (one pad element per 16)
+constexpr int EXN = XH + XH / 16 + 8;  // padded exchange tile (one pad element per 16); +8: the two
+                                       // halves of a line use different banks
 
 __device__ __forceinline__ int padx(int m) { return m + (m >> 4); }
 
@@ -54,7 +55,7 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   __shared__ float2 stw[XP];
   if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int j = lane & 15, h = lane >> 4;
+  const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   float* sin_ = reinterpret_cast<float*>(smraw + wid * xfwd_warp_bytes(a.S));
   float2* sex = reinterpret_cast<float2*>(sin_ + (size_t)a.S * 2 * XH);
   for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   __shared__ float2 stw[XP];
   if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int j = lane & 15, h = lane >> 4;
+  const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   XInvSmem& sm = reinterpret_cast<XInvSmem*>(smraw)[wid];
   for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
   const int npair = (a.rows + 1) >> 1;
@@ -190,16 +191,17 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
       for (int b = 0; b < XR; ++b) v[b] = cmulc(v[b], stw[j + XR * b]);
     }
     __syncwarp();
-    // z[n] = g0[n] + conj(w^n) g1[n]; lanes h = 0 finish n = j + 16 b for b < 8, lanes h = 1 for b >= 8
+    // z[n] = g0[n] + conj(w^n) g1[n]; lanes h = 0 finish n = j + 16 b for even b, lanes h = 1 for odd b
+    // (bank of orow[n]: j + 16 h, all 32 lanes distinct)
     float* orow = reinterpret_cast<float*>(sm.ex);  // [2][256]
 #pragma unroll
     for (int bb = 0; bb < XR / 2; ++bb) {
-      const float2 mine = h ? v[bb + XR / 2] : v[bb];
-      const float2 send = h ? v[bb] : v[bb + XR / 2];
+      const float2 mine = h ? v[2 * bb + 1] : v[2 * bb];
+      const float2 send = h ? v[2 * bb] : v[2 * bb + 1];
       float2 recv;
-      recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
-      recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
-      const int n = j + XR * (h ? bb + XR / 2 : bb);
+      recv.x = __shfl_xor_sync(0xffffffffu, send.x, 1);
+      recv.y = __shfl_xor_sync(0xffffffffu, send.y, 1);
+      const int n = j + XR * (2 * bb + h);
       orow[n] = mine.x + recv.x;
       orow[XH + n] = mine.y + recv.y;
     }
