@@ -514,13 +514,18 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
       const int ko = (yy & 1) ? a.p_outer - ((yy + 1) >> 1) : (yy >> 1);
       const int kx0 = (tile - yy * a.ntile_main) * TL;
       const float2* src = a.spec + (size_t)ko * a.outer_stride + kx0;
-      // 3 H rows of TL float2 = 8 chunks of 16 B each
-      for (int q = threadIdx.x; q < 3 * H * (TL / 2); q += NT) {
-        const int row = q / (TL / 2), ch = q % (TL / 2);
-        const int c = row / H, n = row % H;
-        cpa_zfill<16>(dst + (size_t)row * TL + 2 * ch,
-                      src + (size_t)c * a.comp_stride + (size_t)n * a.line_stride + 2 * ch, n < a.n_valid);
-      }
+      // 3 H rows of TL float2 = 8 chunks of 16 B each; thread t always copies chunk t % 8 of rows
+      // t / 8 + (NT / 8) i: the source offsets are two row offsets x three components
+      constexpr int RPI = NT / (TL / 2);  // rows per sweep of the CTA
+      const int ch = threadIdx.x % (TL / 2), r0 = threadIdx.x / (TL / 2);
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int i = 0; i < H / RPI; ++i) {
+          const int n = r0 + RPI * i;
+          cpa_zfill<16>(dst + (c * H + n) * TL + 2 * ch,
+                        src + (size_t)c * a.comp_stride + (size_t)n * a.line_stride + 2 * ch, n < a.n_valid);
+        }
     } else {
       const int ko0 = (tile - ntm) * TL;
       for (int q = threadIdx.x; q < 3 * H * TL; q += NT) {
@@ -556,14 +561,17 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
     int kom = ko, so = 0;
     if (a.p_outer > 1 && 2 * ko > a.p_outer) { kom = a.p_outer - ko; so = 1; }
     // kernel spectrum of this thread's 8 wave numbers: issued now, used after the forward transform
-    const float* kb = a.khat + (size_t)kom * a.k_outer_stride + kx;
+    // (32-bit element offsets from the uniform base pointer: the launcher checks that they fit)
+    const unsigned kis = (unsigned)a.k_inner_stride, kcs = (unsigned)a.k_comp_stride;
+    const unsigned koff = (unsigned)kom * (unsigned)a.k_outer_stride + (unsigned)kx;
     float K[R][6];
 #pragma unroll
     for (int b = 0; b < R; ++b) {
       const int kz = 2 * (j + R * b) + h;
-      const int pm = 2 * kz > P ? P - kz : kz;
+      const unsigned pm = 2 * kz > P ? P - kz : kz;
+      const unsigned o = koff + pm * kis;
 #pragma unroll
-      for (int c = 0; c < 6; ++c) K[b][c] = __ldg(kb + (size_t)pm * a.k_inner_stride + (size_t)c * a.k_comp_stride);
+      for (int c = 0; c < 6; ++c) K[b][c] = __ldg(a.khat + (o + c * kcs));
     }
     if (nxt < nt) asm volatile("cp.async.wait_group 1;" ::: "memory");
     else asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -573,10 +581,9 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
 #pragma unroll
-      for (int u = 0; u < R; ++u) X[c][u] = xin[(size_t)(c * H + j + R * u) * TL];
-      if (h) {
-#pragma unroll
-        for (int u = 0; u < R; ++u) X[c][u] = cmul(X[c][u], stw[j + R * u]);
+      for (int u = 0; u < R; ++u) {
+        const float2 w = h ? stw[j + R * u] : make_float2(1.f, 0.f);  // (both halves share a warp: no branch)
+        X[c][u] = cmul(xin[(c * H + j + R * u) * TL], w);
       }
       Dft<R, -1>::run(X[c]);
       float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
@@ -616,16 +623,18 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
       for (int q = 1; q < R; ++q) t[(j * R + q) * TL] = cmulc(X[c][q], stw[2 * j * q]);
     }
     __syncthreads();
-    float2* base = a.spec + (size_t)ko * a.outer_stride + kx;
+    const unsigned soff = (unsigned)ko * (unsigned)a.outer_stride + (unsigned)kx;
+    const unsigned sls = (unsigned)a.line_stride, scs = (unsigned)a.comp_stride;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
       const float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
 #pragma unroll
       for (int q = 0; q < R; ++q) X[c][q] = t[(q * R + j) * TL];
       Dft<R, +1>::run(X[c]);
-      if (h) {
 #pragma unroll
-        for (int b = 0; b < R; ++b) X[c][b] = cmulc(X[c][b], stw[j + R * b]);
+      for (int b = 0; b < R; ++b) {
+        const float2 w = h ? stw[j + R * b] : make_float2(1.f, 0.f);
+        X[c][b] = cmulc(X[c][b], w);
       }
 #pragma unroll
       for (int bb = 0; bb < R / 2; ++bb) {
@@ -635,8 +644,7 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
         recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
         recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
         const int n = j + R * (h ? bb + R / 2 : bb);
-        if (ok && n < a.n_valid)
-          base[(size_t)c * a.comp_stride + (size_t)n * a.line_stride] = cadd(mine, recv);
+        if (ok && n < a.n_valid) a.spec[soff + c * scs + (unsigned)n * sls] = cadd(mine, recv);
       }
     }
   }
@@ -1001,6 +1009,8 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   int grid = 2 * w->sm_count;
   if (grid > nt) grid = nt;
   if (L.p_outer != L.n_outer) return mmx_fail(MMX_EINVAL, "inner column pass: outer extent mismatch");
+  if (3 * L.comp_stride >= (1ull << 31) || 6 * L.k_comp_stride >= (1ull << 31))
+    return mmx_fail(MMX_EINVAL, "inner column pass: spectra exceed the 32-bit element offsets of this kernel");
   k_inner_pipe<8><<<grid, 256, smem, w->stream>>>(a);
 #elif MMX_INNER_VARIANT == 1
   const size_t smem = sizeof(float2) * 6 * 64 * TL + sizeof(float) * 6 * 65 * TL;
