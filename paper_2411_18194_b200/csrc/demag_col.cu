@@ -23,6 +23,9 @@ using namespace mmxreg;
 #ifndef MMX_MID_PERSISTENT
 #define MMX_MID_PERSISTENT 1
 #endif
+#ifndef MMX_INNER_TL
+#define MMX_INNER_TL 16       // columns per CTA of variant P (16: two 256-thread CTAs per SM, 207 us on c4; 8: four of 128, 272 us)
+#endif
 #ifndef MMX_MID_PIPE
 #define MMX_MID_PIPE 1        // 1: pipelined y pass (cp.async stages) for 512-point lines on large grids
 #endif
@@ -488,16 +491,18 @@ __device__ __forceinline__ void cpa_zfill(void* smem, const void* gmem, bool val
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(sa), "l"(gmem), "r"(n) : "memory");
 }
 
-template <int R>
-__global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
-  constexpr int H = R * R, P = 2 * H, TL = 16, NT = 32 * R;
+template <int R, int TL>
+__global__ void __launch_bounds__(2 * TL * R, 32 / TL) k_inner_pipe(InnerColArgs a) {
+  constexpr int H = R * R, P = 2 * H, NT = 2 * TL * R;
+  constexpr int EXT = H * TL + (TL < 16 ? 8 : 0);  // one exchange tile (+8: the halves of a 64-bit wavefront use different banks)
   extern __shared__ __align__(16) unsigned char smraw[];
   float2* sm = reinterpret_cast<float2*>(smraw);             // exchange [3][2][H][TL]
-  float2* stage = sm + (size_t)6 * H * TL;                   // input stages [2][3][H][TL]
+  float2* stage = sm + (size_t)6 * EXT;                      // input stages [2][3][H][TL]
   __shared__ float2 stw[P];
   if (a.gated && !a.ctrl->active) return;
-  const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
-  const int kxl = lane & 15, h = lane >> 4;
+  // lane = column + TL h (+ 2 TL (j % (16 / TL)) when TL < 16)
+  const int lane = threadIdx.x & 31;
+  const int kxl = lane % TL, h = (lane / TL) & 1, j = (threadIdx.x >> 5) * (16 / TL) + lane / (2 * TL);
   for (int q = threadIdx.x; q < P; q += NT) stw[q] = a.tw[q];
   const int ntm = a.ntile_main * a.p_outer;
   const int nt = ntm + (a.nyq ? (a.p_outer + TL - 1) / TL : 0);
@@ -586,7 +591,7 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
         X[c][u] = cmul(xin[(c * H + j + R * u) * TL], w);
       }
       Dft<R, -1>::run(X[c]);
-      float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+      float2* t = sm + (c * 2 + h) * EXT + kxl;
       t[(0 * R + j) * TL] = X[c][0];
 #pragma unroll
       for (int q = 1; q < R; ++q) t[(q * R + j) * TL] = cmul(X[c][q], stw[2 * j * q]);
@@ -594,7 +599,7 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
     __syncthreads();
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      const float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+      const float2* t = sm + (c * 2 + h) * EXT + kxl;
 #pragma unroll
       for (int q = 0; q < R; ++q) X[c][q] = t[(j * R + q) * TL];
       Dft<R, -1>::run(X[c]);
@@ -617,7 +622,7 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
       Dft<R, +1>::run(X[c]);
-      float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+      float2* t = sm + (c * 2 + h) * EXT + kxl;
       t[(j * R + 0) * TL] = X[c][0];
 #pragma unroll
       for (int q = 1; q < R; ++q) t[(j * R + q) * TL] = cmulc(X[c][q], stw[2 * j * q]);
@@ -627,7 +632,7 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
     const unsigned sls = (unsigned)a.line_stride, scs = (unsigned)a.comp_stride;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      const float2* t = sm + (size_t)(c * 2 + h) * H * TL + kxl;
+      const float2* t = sm + (c * 2 + h) * EXT + kxl;
 #pragma unroll
       for (int q = 0; q < R; ++q) X[c][q] = t[(q * R + j) * TL];
       Dft<R, +1>::run(X[c]);
@@ -641,8 +646,8 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_pipe(InnerColArgs a) {
         const float2 mine = h ? X[c][bb + R / 2] : X[c][bb];
         const float2 send = h ? X[c][bb] : X[c][bb + R / 2];
         float2 recv;
-        recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
-        recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+        recv.x = __shfl_xor_sync(0xffffffffu, send.x, TL);
+        recv.y = __shfl_xor_sync(0xffffffffu, send.y, TL);
         const int n = j + R * (h ? bb + R / 2 : bb);
         if (ok && n < a.n_valid) a.spec[soff + c * scs + (unsigned)n * sls] = cadd(mine, recv);
       }
@@ -990,7 +995,9 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   InnerColArgs a;
   a.spec = L.spec; a.khat = d.khat; a.tw = L.tw; a.ctrl = w->d_ctrl; a.gated = 1;
   a.n_valid = L.n_valid; a.xc = d.xc; a.p_outer = L.p_outer;
-#if MMX_INNER_VARIANT >= 1
+#if MMX_INNER_VARIANT == 2
+  constexpr int TL = MMX_INNER_TL;
+#elif MMX_INNER_VARIANT == 1
   constexpr int TL = 16;
 #else
   constexpr int TL = 32;
@@ -1003,15 +1010,15 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   a.odd_inner = L.odd_inner; a.odd_outer = L.odd_outer;
   ProfScope ps(w, PK_INNER);
 #if MMX_INNER_VARIANT == 2
-  const size_t smem = sizeof(float2) * (6 + 6) * 64 * TL;
-  if (int rc = set_smem_col(k_inner_pipe<8>, smem)) return rc;
+  const size_t smem = sizeof(float2) * (6 * (64 * TL + (TL < 16 ? 8 : 0)) + 6 * 64 * TL);
+  if (int rc = set_smem_col(k_inner_pipe<8, TL>, smem)) return rc;
   const int nt = a.ntile_main * L.n_outer + (a.nyq ? (L.p_outer + TL - 1) / TL : 0);
-  int grid = 2 * w->sm_count;
+  int grid = (32 / TL) * w->sm_count;
   if (grid > nt) grid = nt;
   if (L.p_outer != L.n_outer) return mmx_fail(MMX_EINVAL, "inner column pass: outer extent mismatch");
   if (3 * L.comp_stride >= (1ull << 31) || 6 * L.k_comp_stride >= (1ull << 31))
     return mmx_fail(MMX_EINVAL, "inner column pass: spectra exceed the 32-bit element offsets of this kernel");
-  k_inner_pipe<8><<<grid, 256, smem, w->stream>>>(a);
+  k_inner_pipe<8, TL><<<grid, 2 * TL * 8, smem, w->stream>>>(a);
 #elif MMX_INNER_VARIANT == 1
   const size_t smem = sizeof(float2) * 6 * 64 * TL + sizeof(float) * 6 * 65 * TL;
   if (int rc = set_smem_col(k_inner_w<8>, smem)) return rc;
