@@ -37,13 +37,20 @@ def test_dp45_fixed_step_trajectory(name, grid, nsteps):
     spec = wl.make(name, grid)
     dt = spec.integrator["dt"]
     g, o = pair(spec)
+    bmax = max(float(np.sqrt((o.heff(s) ** 2).sum(axis=0)).max()) for s in range(spec.S))
     st = g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=nsteps)
     errs = o.step_dp45_fixed(dt, nsteps)
     assert st["accepted"] == nsteps and st["rejected"] == 0
     _compare_state(g, o, spec)
     hist = g.get_err_history(nsteps)
     assert len(hist) == nsteps
-    np.testing.assert_allclose(hist, errs, rtol=2e-2, atol=1e-9)
+    # fp32 floor of the estimate dt |sum_j e_j k_j|: the torque m x B is formed in fp32 from a field
+    # that is nearly parallel to m (33 T of inter-sublattice exchange in c5), so each k_j carries an
+    # absolute rounding error of about gamma max|B_eff| 2^-24 per operation, ~16 operations deep, and
+    # the combination weights it with sum_j |e_j| = 0.16 (Dormand-Prince, Table 2):
+    #   atol = 16 * 2^-24 * 0.16 * dt * gamma * max|B_eff|
+    atol = 16 * 2.0 ** -24 * 0.16 * dt * 1.7595e11 * bmax
+    np.testing.assert_allclose(hist, errs, rtol=2e-2, atol=max(atol, 1e-9))
     if spec.elastic is not None:
         u, v = g.get_state(mmx.F_U), g.get_state(mmx.F_V)
         assert np.abs(u - o.u).max() <= 1e-4 * max(np.abs(o.u).max(), 1e-30)
