@@ -34,7 +34,7 @@ DT = {"c1": 1e-13, "c2": 2e-14, "c3": 5e-15, "c4": 1e-13, "c5": 5e-15}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
 # committed `ncu --set full` capture (profiles/, see the .md beside it); None until captured.
-NCU_TRAFFIC_BYTES = {"demag_inner": None}
+NCU_TRAFFIC_BYTES = {"demag_inner": 339184896 + 170884096}  # profiles/ncu_r1_kernels.md (k_inner_pipe<8,16>)
 
 
 def measured_peaks():
@@ -90,7 +90,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -284,10 +284,11 @@ def run_mmx(args, rank, local_rank, world_size):
     cpu = None
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
         grid = oracle_sample_grid(name, 1)
-        v, s_step = time_oracle(name, grid, 1, 1)
+        nstep_cpu = 5  # about 12 s of CPU work on the c4 sample box
+        v, s_step = time_oracle(name, grid, nstep_cpu, 1)
         cpu = {"value": v, "unit": UNIT, "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
-               "sample": "1 fixed-step DP45 step of the fp64 numpy oracle on a %dx%dx%d box of the %s recipe "
-                         "(%.1f s)" % (*grid, name, s_step)}
+               "sample": "%d fixed-step DP45 steps of the fp64 numpy oracle on a %dx%dx%d box of the %s recipe "
+                         "(%.1f s per step)" % (nstep_cpu, *grid, name, s_step)}
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": K, "warmup": W,
@@ -308,7 +309,7 @@ def run_mmx(args, rank, local_rank, world_size):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="mmx", choices=["mmx", "reference"])
     ap.add_argument("--config", default="c4", choices=list(DT))
