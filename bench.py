@@ -81,7 +81,7 @@ def algorithmic_bytes(spec):
 
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled during the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -95,7 +95,19 @@ class ClockSampler:
         except OSError:
             self.p = None
 
-    def stop(self):
+    def wait_first_sample(self, timeout=3.0):
+        """nvidia-smi needs ~0.1-0.3 s before its first line: call before the timed region."""
+        t0 = time.time()
+        while self.p is not None and time.time() - t0 < timeout:
+            if os.path.getsize(self.f.name) > 0:
+                return
+            time.sleep(0.01)
+
+    def mark(self):
+        return time.time()
+
+    def stop(self, t_begin=None, t_end=None):
+        import datetime
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
         if self.p is None:
             return out
@@ -110,8 +122,16 @@ class ClockSampler:
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f.read().splitlines():
             c = [x.strip() for x in line.split(",")]
-            if len(c) < 8:
+            if len(c) < 9:
                 continue
+            if t_begin is not None:
+                try:
+                    ts = datetime.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                except ValueError:
+                    continue
+                if ts < t_begin - 0.02 or ts > t_end + 0.02:   # keep samples taken under load
+                    continue
+            c = c[1:]
             try:
                 sm.append(float(c[0])); mx.append(float(c[1]))
             except ValueError:
@@ -211,16 +231,20 @@ def run_mmx(args, rank, local_rank, world_size):
             dist.barrier()
             torch.cuda.synchronize()
 
-    steps(W)
     clocks = ClockSampler(local_rank) if rank == 0 else None
+    steps(W)
+    if clocks:
+        clocks.wait_first_sample()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    t_begin = time.time()
     e0.record(stream)
     st = steps(K)
     e1.record(stream)
     barrier()
+    t_end = time.time()
     ms = e0.elapsed_time(e1)
-    clk = clocks.stop() if clocks else None
+    clk = clocks.stop(t_begin, t_end) if clocks else None
     if dist is not None:
         t = torch.tensor([ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
