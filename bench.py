@@ -194,6 +194,21 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(ms, dist, device):
+    """Replicas only: the job time is the slowest rank's device time."""
+    if dist is None:
+        return ms
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_seed(name, rank, world_size):
+    """Every rank integrates an independent world of the same recipe (weak scaling)."""
+    return None if world_size == 1 else 1000 + int(name[1]) + 100 * rank
+
+
 def run_mmx(args, rank, local_rank, world_size):
     import torch
 
@@ -213,9 +228,8 @@ def run_mmx(args, rank, local_rank, world_size):
         dist.barrier()
 
     name = args.config
-    spec = wl.make(name)                      # every rank: an independent replica, same recipe
-    if world_size > 1:
-        spec = wl.make(name, seed=1000 + int(name[1]) + 100 * rank)
+    seed = replica_seed(name, rank, world_size)   # every rank: an independent replica, same recipe
+    spec = wl.make(name) if seed is None else wl.make(name, seed=seed)
     N = spec.ncells
     stream = torch.cuda.current_stream()
     g = mmx.World.from_spec(spec, stream=stream.cuda_stream)
@@ -245,10 +259,7 @@ def run_mmx(args, rank, local_rank, world_size):
     t_end = time.time()
     ms = e0.elapsed_time(e1)
     clk = clocks.stop(t_begin, t_end) if clocks else None
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, "cuda")
     value = N * K * world_size / (ms * 1e-3)
     launches = int(st["launches"])
 
