@@ -547,6 +547,11 @@ __global__ void __launch_bounds__(2 * TL * R, 32 / TL) k_inner_pipe(InnerColArgs
 
   int tile = blockIdx.x;
   if (tile < nt) issue(tile, 0);
+#ifdef MMX_INNER_STAGGER_NS
+  // the CTAs that share an SM would otherwise run the same phase (butterflies / exchange) at the same
+  // time for the whole kernel; delay the second wave by about half a tile
+  if (blockIdx.x >= gridDim.x / 2) __nanosleep(MMX_INNER_STAGGER_NS);
+#endif
   int buf = 0;
   for (; tile < nt; tile += gridDim.x, buf ^= 1) {
     const int nxt = tile + gridDim.x;

@@ -227,3 +227,20 @@ def test_c4_full_size_sampled_against_direct_sum():
     e = field_err(g.eval_heff(0, mmx.T_EXCH), o.field_terms(0, terms=oc.T_EXCH)[oc.T_EXCH])
     assert e < FIELD_TOL, e
     g.destroy()
+
+
+@pytest.mark.parametrize("name,grid", [("c1", (64, 40, 1)), ("c1", (256, 64, 1)), ("c2", (256, 128, 1))])
+def test_fast_path_two_dimensional_worlds(name, grid):
+    """2-D worlds whose innermost transformed axis (y, 128 points) takes the fused column pass and,
+    for Nx = 256, the warp x passes; c2 is periodic (no pruning: generic passes) with the float4
+    local kernel on periodic stencils."""
+    spec = _rich_spec(name, grid, seed=13)
+    g, o = pair(spec)
+    ref = o.field_terms(0)
+    for tname in ("demag", "exch", "dmi", "anis_u"):
+        bit = TERMS[tname]
+        e = field_err(g.eval_heff(0, bit), ref[bit])
+        assert e < FIELD_TOL, (name, grid, tname, e)
+    e = field_err(g.eval_torque(0), o.torque(0))
+    assert e < FIELD_TOL, (name, grid, "torque", e)
+    g.destroy()
