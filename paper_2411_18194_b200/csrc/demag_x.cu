@@ -50,24 +50,27 @@ struct XWArgs {
 // then float2 ex[2 * EXN] (exchange tiles of the two halves; reused as Z[512])
 __host__ __device__ inline size_t xfwd_warp_bytes(int S) { return (size_t)S * 2 * XH * sizeof(float) + 2 * EXN * sizeof(float2); }
 
+// FULL: Nx = 256, an even number of rows, one sublattice (the c4 shape): sizes become constants
+template <bool FULL>
 __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
+  const int nx = FULL ? XH : a.nx, S = FULL ? 1 : a.S;
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ float2 stw[XP];
   if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
-  float* sin_ = reinterpret_cast<float*>(smraw + wid * xfwd_warp_bytes(a.S));
-  float2* sex = reinterpret_cast<float2*>(sin_ + (size_t)a.S * 2 * XH);
+  float* sin_ = reinterpret_cast<float*>(smraw + wid * xfwd_warp_bytes(S));
+  float2* sex = reinterpret_cast<float2*>(sin_ + (size_t)S * 2 * XH);
   for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
-  const float* y = a.yin[a.ctrl->sel];
+  const float* y = a.ctrl->sel ? a.yin[1] : a.yin[0];  // (no dynamic index into the parameter block)
   const int npair = (a.rows + 1) >> 1;
   const int nwarp = gridDim.x * XW;
-  const int chunks = a.nx >> 1;  // 16-byte chunks of a row pair: 2 nx floats / 4
+  const int chunks = nx >> 1;  // 16-byte chunks of a row pair: 2 nx floats / 4
 
   auto prefetch = [&](int pair) {
-    for (int s = 0; s < a.S; ++s) {
-      const float* src = y + (size_t)s * 3 * a.N + (size_t)pair * 2 * a.nx;
-      const bool full = 2 * pair + 1 < a.rows;
+    for (int s = 0; s < S; ++s) {
+      const float* src = y + (size_t)s * 3 * a.N + (size_t)pair * 2 * nx;
+      const bool full = FULL || 2 * pair + 1 < a.rows;
       for (int c = lane; c < chunks; c += 32)
         if (full || 2 * c < chunks) cp16(sin_ + s * 2 * XH + 4 * c, src + 4 * c);
     }
@@ -80,27 +83,28 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   for (; pair < npair; pair += nwarp) {
     cp_wait<0>();
     __syncwarp();
-    const bool two = 2 * pair + 1 < a.rows;
+    const bool two = FULL || 2 * pair + 1 < a.rows;
     float2 v[XR];
 #pragma unroll
     for (int u = 0; u < XR; ++u) {
       const int n = j + XR * u;
       float ra = 0.f, rb = 0.f;
-      if (n < a.nx) {
+      if (FULL || n < nx) {
         ra = a.ms[0] * sin_[n];
-        rb = two ? a.ms[0] * sin_[a.nx + n] : 0.f;
-        if (a.S == 2) {
+        rb = two ? a.ms[0] * sin_[nx + n] : 0.f;
+        if (S == 2) {
           ra = fmaf(a.ms[1], sin_[2 * XH + n], ra);
-          if (two) rb = fmaf(a.ms[1], sin_[2 * XH + a.nx + n], rb);
+          if (two) rb = fmaf(a.ms[1], sin_[2 * XH + nx + n], rb);
         }
       }
       v[u] = make_float2(ra, rb);
     }
     __syncwarp();
     if (pair + nwarp < npair) prefetch(pair + nwarp);  // overlaps the transform below
-    if (h) {
 #pragma unroll
-      for (int u = 0; u < XR; ++u) v[u] = cmul(v[u], stw[j + XR * u]);
+    for (int u = 0; u < XR; ++u) {
+      const float2 w = h ? stw[j + XR * u] : make_float2(1.f, 0.f);  // (both halves share a warp: no branch)
+      v[u] = cmul(v[u], w);
     }
     Dft<XR, -1>::run(v);
     float2* ex = sex + h * EXN;
@@ -136,7 +140,9 @@ struct __align__(16) XInvSmem {
   float2 ex[2 * EXN];         // exchange tiles; reused as the two output rows [2][256] floats
 };
 
+template <bool FULL>
 __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
+  const int nx = FULL ? XH : a.nx;
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ float2 stw[XP];
   if (a.gated && !a.ctrl->active) return;
@@ -149,7 +155,7 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   constexpr int CH = (XH + 1 + 1) / 2;  // 16-byte chunks covering 257 complex values
 
   auto prefetch = [&](int pair) {
-    const bool two = 2 * pair + 1 < a.rows;
+    const bool two = FULL || 2 * pair + 1 < a.rows;
     for (int r = 0; r < (two ? 2 : 1); ++r) {
       const float2* src = a.spec + (size_t)(2 * pair + r) * a.xp;
       for (int c = lane; c < CH; c += 32) cp16(&sm.in[r][2 * c], src + 2 * c);
@@ -163,7 +169,7 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   for (; pair < npair; pair += nwarp) {
     cp_wait<0>();
     __syncwarp();
-    const bool two = 2 * pair + 1 < a.rows;
+    const bool two = FULL || 2 * pair + 1 < a.rows;
     const float2* A = sm.in[0];
     const float2* B = sm.in[1];
     float2 v[XR];
@@ -186,9 +192,10 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
 #pragma unroll
     for (int q = 0; q < XR; ++q) v[q] = ex[padx(j * XR + q)];
     Dft<XR, +1>::run(v);
-    if (h) {
 #pragma unroll
-      for (int b = 0; b < XR; ++b) v[b] = cmulc(v[b], stw[j + XR * b]);
+    for (int b = 0; b < XR; ++b) {
+      const float2 w = h ? stw[j + XR * b] : make_float2(1.f, 0.f);
+      v[b] = cmulc(v[b], w);
     }
     __syncwarp();
     // z[n] = g0[n] + conj(w^n) g1[n]; lanes h = 0 finish n = j + 16 b for even b, lanes h = 1 for odd b
@@ -206,10 +213,10 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
       orow[XH + n] = mine.y + recv.y;
     }
     __syncwarp();
-    float* o0 = a.bout + (size_t)(2 * pair) * a.nx;
-    for (int c = lane; c < (a.nx >> 2); c += 32) {
+    float* o0 = a.bout + (size_t)(2 * pair) * nx;
+    for (int c = lane; c < (nx >> 2); c += 32) {
       *reinterpret_cast<float4*>(o0 + 4 * c) = *reinterpret_cast<const float4*>(orow + 4 * c);
-      if (two) *reinterpret_cast<float4*>(o0 + a.nx + 4 * c) = *reinterpret_cast<const float4*>(orow + XH + 4 * c);
+      if (two) *reinterpret_cast<float4*>(o0 + nx + 4 * c) = *reinterpret_cast<const float4*>(orow + XH + 4 * c);
     }
     __syncwarp();  // the output rows alias the exchange tiles of the next iteration
   }
@@ -235,16 +242,27 @@ int mmx_x_warp_launch(mmx_world* w, int dir, const float* const yin[2], float* b
   const int npair = (a.rows + 1) / 2;
   int blocks = (dir < 0 ? 4 : 3) * w->sm_count;
   if (blocks * XW > npair) blocks = (npair + XW - 1) / XW;
+  const bool full = d.nx == XH && (a.rows & 1) == 0 && w->S == 1;
   if (dir < 0) {
     const size_t smem = xfwd_warp_bytes(a.S) * XW;
-    MMX_CUDA(cudaFuncSetAttribute(k_x_fwd_w, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ProfScope ps(w, PK_X_FWD);
-    k_x_fwd_w<<<blocks, 32 * XW, smem, w->stream>>>(a);
+    if (full) {
+      MMX_CUDA(cudaFuncSetAttribute(k_x_fwd_w<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k_x_fwd_w<true><<<blocks, 32 * XW, smem, w->stream>>>(a);
+    } else {
+      MMX_CUDA(cudaFuncSetAttribute(k_x_fwd_w<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k_x_fwd_w<false><<<blocks, 32 * XW, smem, w->stream>>>(a);
+    }
   } else {
     const size_t smem = sizeof(XInvSmem) * XW;
-    MMX_CUDA(cudaFuncSetAttribute(k_x_inv_w, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ProfScope ps(w, PK_X_INV);
-    k_x_inv_w<<<blocks, 32 * XW, smem, w->stream>>>(a);
+    if (full) {
+      MMX_CUDA(cudaFuncSetAttribute(k_x_inv_w<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k_x_inv_w<true><<<blocks, 32 * XW, smem, w->stream>>>(a);
+    } else {
+      MMX_CUDA(cudaFuncSetAttribute(k_x_inv_w<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k_x_inv_w<false><<<blocks, 32 * XW, smem, w->stream>>>(a);
+    }
   }
   MMX_CUDA(cudaGetLastError());
   return MMX_OK;
