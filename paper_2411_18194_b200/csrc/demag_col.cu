@@ -890,12 +890,16 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
     if (tile < ntm) {
       const int slab = tile / a.ntile_main;
       const int kx0 = (tile - slab * a.ntile_main) * TL;
-      const float2* src = a.in + (size_t)slab * a.in_outer + kx0;
+      // thread t always copies 16-byte chunk t % 4 of rows t / 4 + (NT / 4) i; 32-bit element offsets
+      // from the uniform base (the launcher checks that they fit)
+      constexpr int RPI = NT / (TL / 2);
+      const unsigned ch = threadIdx.x % (TL / 2), r0 = threadIdx.x / (TL / 2);
+      const unsigned xp = (unsigned)a.xp;
+      const unsigned so = (unsigned)slab * (unsigned)a.in_outer + (unsigned)kx0 + r0 * xp + 2 * ch;
 #pragma unroll
-      for (int q0 = 0; q0 < ROWS * (TL / 2); q0 += NT) {
-        const int q = q0 + threadIdx.x;
-        const int row = q / (TL / 2), ch = q % (TL / 2);
-        cpa_zfill<16>(dst + row * TL + 2 * ch, src + (size_t)row * a.xp + 2 * ch, row < a.n_in);
+      for (int i = 0; i < ROWS / RPI; ++i) {
+        const int row = r0 + RPI * i;
+        cpa_zfill<16>(dst + row * TL + 2 * ch, a.in + (so + (unsigned)(RPI * i) * xp), row < a.n_in);
       }
     } else {
       const int slab0 = (tile - ntm) * TL;
@@ -952,11 +956,13 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
 #pragma unroll
     for (int q = 0; q < R; ++q) v[q] = ex[(j * R + q) * TL];
     Dft<R, DIR>::run(v);
-    float2* out = a.out + (size_t)slab * a.out_outer + kx;
+    const unsigned xpu = (unsigned)a.xp;
+    const unsigned oo = (unsigned)slab * (unsigned)a.out_outer + (unsigned)kx;
     if (DIR < 0) {
       if (ok) {
+        const unsigned o0 = oo + (unsigned)(2 * j + h) * xpu;
 #pragma unroll
-        for (int b = 0; b < R; ++b) out[(size_t)(2 * (j + R * b) + h) * a.xp] = v[b];
+        for (int b = 0; b < R; ++b) a.out[o0 + (unsigned)(2 * R * b) * xpu] = v[b];
       }
     } else {
       // x[n] = g0[n] + conj(w_P^n) g1[n]: lanes h = 0 finish rows b < R/2, lanes h = 1 the others
@@ -973,7 +979,7 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
         recv.x = __shfl_xor_sync(0xffffffffu, send.x, 8);
         recv.y = __shfl_xor_sync(0xffffffffu, send.y, 8);
         const int n = j + R * (h ? bb + R / 2 : bb);
-        if (ok && n < a.n_out) out[(size_t)n * a.xp] = cadd(mine, recv);
+        if (ok && n < a.n_out) a.out[oo + (unsigned)n * xpu] = cadd(mine, recv);
       }
     }
   }
@@ -1059,7 +1065,8 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
   // measured on c4: the register-prefetching persistent form wins for the inverse pass (89 vs 95 us),
   // the plain grid for the forward pass (80 vs 90 us)
 #if MMX_MID_PIPE
-  if (R == 16 && ntiles >= 8 * w->sm_count) {
+  if (R == 16 && ntiles >= 8 * w->sm_count && (size_t)a.nslab * a.out_outer < (1ull << 31) &&
+      (size_t)a.nslab * a.in_outer < (1ull << 31)) {
     MidColArgs b = a;
     constexpr int TL = 8;
     b.nyq = ((a.xc - 1) % TL == 0 && a.xc > 1 && a.nslab >= TL) ? 1 : 0;
