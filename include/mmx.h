@@ -145,7 +145,10 @@ const char* mmx_version(void);
  *   pbc[3]      = number of periodic image repetitions per axis used by the demag kernel;
  *                 0 = open axis.  A periodic axis must have a power-of-two size.
  *   n_sublattices = 1 (ferromagnet) or 2 (antiferro-/ferrimagnet)
- *   cuda_stream = cudaStream_t (as void*) on which all work is enqueued, or NULL
+ *   cuda_stream = cudaStream_t (as void*) on which all work is enqueued.  NULL: the library
+ *                 creates its own blocking stream (the legacy default stream cannot be captured
+ *                 into the step graph); the runtime orders that stream against the legacy default
+ *                 stream in both directions, so work the caller enqueues on stream 0 keeps its order.
  * Materials default to Ms = 0 everywhere until mmx_set_material is called. */
 int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[3],
                      int n_sublattices, void* cuda_stream, mmx_world** out);
@@ -231,6 +234,15 @@ int mmx_profile_read(mmx_world* w, double* ms_out, long long* count_out, int n);
 
 /* Number of device bytes owned by the world. */
 int mmx_device_bytes(mmx_world* w, long long* bytes);
+
+/* CUDA-graph stepping.  mmx_step_rk4 / mmx_step_rk45 capture one attempt of a step (every kernel of
+ * the step-size controller, the demag passes, the local and elastic kernels) as a CUDA graph on first
+ * use and replay it per attempt; the graph is rebuilt after any mmx_set_* / mmx_enable_demag /
+ * mmx_demag_kernel_init call and is bypassed while the profiler is on.  mmx_graph_enable(w, 0)
+ * switches to plain launches (also: environment variable MMX_NO_GRAPH at world creation).
+ * mmx_graph_info: *kernels_per_replay = kernels inside the instantiated graph, 0 if none is live. */
+int mmx_graph_enable(mmx_world* w, int on);
+int mmx_graph_info(mmx_world* w, long long* kernels_per_replay);
 
 #ifdef __cplusplus
 }

@@ -97,6 +97,8 @@ PROTOTYPES = {
     "mmx_profile_enable": (C.c_int, [_W, C.c_int]),
     "mmx_profile_read": (C.c_int, [_W, _D3, C.POINTER(C.c_longlong), C.c_int]),
     "mmx_device_bytes": (C.c_int, [_W, C.POINTER(C.c_longlong)]),
+    "mmx_graph_enable": (C.c_int, [_W, C.c_int]),
+    "mmx_graph_info": (C.c_int, [_W, C.POINTER(C.c_longlong)]),
 }
 
 _lib = None
@@ -329,6 +331,15 @@ class World:
     def device_bytes(self):
         b = C.c_longlong()
         _check(self.lib.mmx_device_bytes(self.h, C.byref(b)))
+        return b.value
+
+    def graph_enable(self, on=True):
+        _check(self.lib.mmx_graph_enable(self.h, 1 if on else 0))
+
+    def graph_info(self):
+        """Kernels inside the live step graph (0: stepping uses plain launches)."""
+        b = C.c_longlong()
+        _check(self.lib.mmx_graph_info(self.h, C.byref(b)))
         return b.value
 
     # ---- convenience: marshal a workloads.WorldSpec (plain data) through the calls above

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstddef>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -205,6 +206,7 @@ int alloc_state(mmx_world* w) {
     if (int rc = dev_alloc(w, &w->strain, 6 * w->N)) return rc;
   w->sel_host = 0;
   w->k1_valid = false;
+  w->cfg_epoch++;
   // ctrl->sel must follow
   int zero = 0;
   MMX_CUDA(cudaMemcpyAsync(&w->d_ctrl->sel, &zero, sizeof(int), cudaMemcpyHostToDevice, w->stream));
@@ -410,6 +412,40 @@ int run_steps(mmx_world* w, const mmx_rk_opts* o, mmx_rk_stats* stats) {
     return mmx_controller_launch(w, tab, 1);
   };
 
+  // One attempt = one CUDA graph launch.  Captured on first use per (method, configuration epoch);
+  // any failure to capture falls back to plain launches.  Off while the per-kernel profiler runs.
+  auto attempt_fast = [&]() -> int {
+    if (!w->use_graphs || w->prof) return attempt();
+    if (!(w->step_graph && w->graph_method == o->method && w->graph_epoch == w->cfg_epoch)) {
+      if (w->step_graph) { cudaGraphExecDestroy(w->step_graph); w->step_graph = nullptr; }
+      const long long l0 = w->launches;
+      cudaGraph_t graph = nullptr;
+      if (cudaStreamBeginCapture(w->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        w->use_graphs = false;
+        return attempt();
+      }
+      const int rc = attempt();
+      const cudaError_t ce = cudaStreamEndCapture(w->stream, &graph);
+      w->graph_launches = w->launches - l0;
+      w->launches = l0;
+      if (rc != MMX_OK || ce != cudaSuccess || graph == nullptr ||
+          cudaGraphInstantiate(&w->step_graph, graph, 0) != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        w->step_graph = nullptr;
+        w->use_graphs = false;
+        return rc != MMX_OK ? rc : attempt();
+      }
+      cudaGraphDestroy(graph);
+      w->graph_method = o->method;
+      w->graph_epoch = w->cfg_epoch;
+    }
+    MMX_CUDA(cudaGraphLaunch(w->step_graph, w->stream));
+    w->launches += w->graph_launches;
+    return MMX_OK;
+  };
+
   const long long max_attempts = o->max_attempts > 0 ? o->max_attempts : 1000000;
   long long done = 0;
   while (done < max_attempts) {
@@ -420,7 +456,7 @@ int run_steps(mmx_world* w, const mmx_rk_opts* o, mmx_rk_stats* stats) {
     if (chunk > 4096) chunk = 4096;
     if (chunk <= 0) break;
     for (long long q = 0; q < chunk; ++q)
-      if (int rc = attempt()) return rc;
+      if (int rc = attempt_fast()) return rc;
     done += chunk;
     if (int rc = read_ctrl(w, &h)) return rc;
     if (!h.active) break;
@@ -499,6 +535,16 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
   w->nvec = w->S;
   w->N = (size_t)grid[0] * grid[1] * grid[2];
   w->stream = (cudaStream_t)cuda_stream;
+  w->own_stream = false;
+  if (!w->stream) {
+    // The legacy default stream cannot be captured into a CUDA graph.  A world created on it runs on
+    // its own *blocking* stream instead, which the runtime orders against the legacy default stream
+    // in both directions, so callers that enqueue on stream 0 see the same ordering as before.
+    if (cudaStreamCreate(&w->stream) == cudaSuccess) w->own_stream = true;
+    else { cudaGetLastError(); w->stream = nullptr; }
+  }
+  w->step_graph = nullptr; w->graph_method = -1; w->graph_epoch = -1; w->cfg_epoch = 0; w->graph_launches = 0;
+  w->use_graphs = getenv("MMX_NO_GRAPH") == nullptr;
   {
     int dev = 0;
     cudaGetDevice(&dev);
@@ -556,6 +602,8 @@ int mmx_world_destroy(mmx_world* w) {
   cudaFree(w->bdemag); cudaFree(w->strain); cudaFree(w->scratch);
   for (int a = 0; a < 3; ++a) cudaFree(w->dm.tw[a]);
   cudaFree(w->dm.spec1); cudaFree(w->dm.spec2); cudaFree(w->dm.khat);
+  if (w->step_graph) cudaGraphExecDestroy(w->step_graph);
+  if (w->own_stream) cudaStreamDestroy(w->stream);
   cudaGetLastError();
   delete w;
   return MMX_OK;
@@ -586,6 +634,7 @@ int mmx_set_regions(mmx_world* w, const uint16_t* region_of_cell, int mem, int n
     MMX_CUDA(cudaStreamSynchronize(w->stream));
   }
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;
 }
 
@@ -597,6 +646,7 @@ int mmx_set_material(mmx_world* w, int sublattice, int region, const mmx_materia
   w->mats[(size_t)sublattice * w->nreg + region] = *mat;
   w->mat_dirty = true;
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;
 }
 
@@ -605,6 +655,7 @@ int mmx_set_coupling(mmx_world* w, const mmx_coupling* c) {
   if (c->A0 != 0.0 && !(c->latcon > 0)) return mmx_fail(MMX_EINVAL, "A0 != 0 needs latcon > 0");
   w->cpl = *c;
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;
 }
 
@@ -612,6 +663,7 @@ int mmx_set_bext(mmx_world* w, const double B[3]) {
   if (!w || !B) return mmx_fail(MMX_EINVAL, "NULL argument");
   for (int a = 0; a < 3; ++a) w->bext[a] = B[a];
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;
 }
 
@@ -619,6 +671,7 @@ int mmx_set_current(mmx_world* w, const double J[3]) {
   if (!w || !J) return mmx_fail(MMX_EINVAL, "NULL argument");
   for (int a = 0; a < 3; ++a) w->J[a] = J[a];
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;
 }
 
@@ -633,6 +686,7 @@ int mmx_set_elastic(mmx_world* w, const mmx_elastic* e) {
     w->has_elastic = false;
   }
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   if (w->Y[0]) return alloc_state(w);
   return MMX_OK;
 }
@@ -641,6 +695,7 @@ int mmx_enable_demag(mmx_world* w, int on) {
   if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
   w->use_demag = on != 0;
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;
 }
 
@@ -756,6 +811,7 @@ int mmx_demag_kernel_init(mmx_world* w, double analytic_cutoff_cells) {
   MMX_CUDA(cudaMemcpy(d.khat, khat.data(), khat.size() * sizeof(float), cudaMemcpyHostToDevice));
   d.ready = true;
   w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;
 }
 
@@ -937,6 +993,18 @@ int mmx_profile_read(mmx_world* w, double* ms_out, long long* count_out, int n) 
 int mmx_device_bytes(mmx_world* w, long long* bytes) {
   if (!w || !bytes) return mmx_fail(MMX_EINVAL, "NULL argument");
   *bytes = w->dev_bytes;
+  return MMX_OK;
+}
+
+int mmx_graph_enable(mmx_world* w, int on) {
+  if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
+  w->use_graphs = on != 0;
+  return MMX_OK;
+}
+
+int mmx_graph_info(mmx_world* w, long long* kernels_per_replay) {
+  if (!w || !kernels_per_replay) return mmx_fail(MMX_EINVAL, "NULL argument");
+  *kernels_per_replay = (w->step_graph && w->graph_epoch == w->cfg_epoch) ? w->graph_launches : 0;
   return MMX_OK;
 }
 

@@ -140,6 +140,7 @@ struct mmx_world {
   int nvec;            // S (+2 with elastic)
   size_t N;
   cudaStream_t stream;
+  bool own_stream;     // created by the library because the caller passed the legacy default stream
   int sm_count;        // multiprocessors of the device (grid size of the persistent kernels)
   int nreg;
   uint16_t* d_reg;
@@ -168,6 +169,14 @@ struct mmx_world {
   long long launches;
   bool prof;
   std::vector<ProfRec> prof_recs;
+  // one attempt of an RK step captured as a CUDA graph (api.cu): every kernel argument of an attempt
+  // is fixed between configuration changes (the "sel pairs" and the device-side controller were
+  // designed for this), so a step is one graph launch instead of 27-39 kernel launches
+  cudaGraphExec_t step_graph;
+  int graph_method;
+  long long graph_epoch, cfg_epoch;   // the graph is valid while graph_epoch == cfg_epoch
+  long long graph_launches;           // kernels per replay
+  bool use_graphs;
 };
 
 // RAII: brackets one kernel launch with CUDA events on the world's stream when profiling is on

@@ -141,3 +141,26 @@ def test_macrospin_closed_form_every_tableau(method, order):
     ref = np.tanh(alpha * gamma * B * T / (1 + alpha ** 2) + np.arctanh(0.5))
     assert np.abs(mz - ref).max() < 2e-5
     g.destroy()
+
+
+def test_graph_replay_equals_plain_launches_and_follows_parameter_changes():
+    """A step is replayed as a CUDA graph; the result must be bit-identical to plain launches, and a
+    parameter change between two stepping calls must rebuild the graph (kernel arguments are baked in)."""
+    spec = wl.make("c2", (32, 32, 1))
+    dt = spec.integrator["dt"]
+    a = mmx.World.from_spec(spec)
+    b = mmx.World.from_spec(spec)
+    b.graph_enable(False)
+    for w in (a, b):
+        w.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=7)
+    assert a.graph_info() > 0 and b.graph_info() == 0
+    assert np.array_equal(a.get_state(mmx.F_M0), b.get_state(mmx.F_M0))
+    for w in (a, b):
+        w.set_bext((0.05, -0.3, 0.2))
+    assert a.graph_info() == 0          # stale: rebuilt on the next stepping call
+    for w in (a, b):
+        w.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=7)
+        w.step_rk4(dt, 3)
+    assert a.graph_info() > 0
+    assert np.array_equal(a.get_state(mmx.F_M0), b.get_state(mmx.F_M0))
+    a.destroy(); b.destroy()
