@@ -30,7 +30,7 @@ using namespace mmxreg;
 #define MMX_MID_PIPE 1        // 1: pipelined y pass (cp.async stages) for 512-point lines on large grids
 #endif
 #ifndef MMX_INNER_VARIANT
-#define MMX_INNER_VARIANT 2   // 2: variant P (persistent, cp.async pipeline); 0: 32-column tiles (persistent when large), 1: variant W (16 columns, halves in one warp)
+#define MMX_INNER_VARIANT 3   // 3: variant Q (kernel rows staged in shared memory, twiddles in registers: 170 us on c4); 2: variant P (persistent, cp.async pipeline, kernel values in registers: 207 us); 0: 32-column tiles (persistent when large), 1: variant W (16 columns, halves in one warp)
 #endif
 
 namespace {
@@ -660,6 +660,184 @@ __global__ void __launch_bounds__(2 * TL * R, 32 / TL) k_inner_pipe(InnerColArgs
   }
 }
 
+// Variant Q of the fused inner pass: as variant P, but the kernel-spectrum rows of a tile are staged
+// in shared memory by cp.async (one tile ahead) instead of being held in 48 registers, and the
+// registers freed hold the 15 twiddles of the thread for the whole kernel (no per-component reloads,
+// no selects).  One spectrum stage (refilled as soon as the tile has been read) + one kernel stage.
+template <int R>
+__global__ void __launch_bounds__(32 * R, 2) k_inner_q(InnerColArgs a) {
+  constexpr int H = R * R, P = 2 * H, TL = 16, NT = 32 * R, EXT = H * TL;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  float2* sm = reinterpret_cast<float2*>(smraw);             // exchange [3][2][H][TL]
+  float2* xst = sm + 6 * EXT;                                // spectrum stage [3][H][TL]
+  float* kst = reinterpret_cast<float*>(xst + 3 * H * TL);   // kernel stage [6][H+1][TL]
+  if (a.gated && !a.ctrl->active) return;
+  const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
+  const int kxl = lane & 15, h = lane >> 4;
+  const int ntm = a.ntile_main * a.p_outer;
+  const int nt = ntm + (a.nyq ? (a.p_outer + TL - 1) / TL : 0);
+  // twiddles of this thread: stage w_H^(j q), half w_P^(j + R u) (identity for the even half)
+  float2 tws[R], twp[R];
+#pragma unroll
+  for (int q = 0; q < R; ++q) {
+    tws[q] = a.tw[2 * j * q];
+    twp[q] = h ? a.tw[j + R * q] : make_float2(1.f, 0.f);
+  }
+
+  auto tile_ko = [&](int tile) -> int {
+    const int yy = tile / a.ntile_main;
+    return (yy & 1) ? a.p_outer - ((yy + 1) >> 1) : (yy >> 1);
+  };
+  auto issue_x = [&](int tile) {
+    if (tile < ntm) {
+      const int ko = tile_ko(tile);
+      const int kx0 = (tile - (tile / a.ntile_main) * a.ntile_main) * TL;
+      constexpr int RPI = NT / (TL / 2);
+      const unsigned ch = threadIdx.x % (TL / 2), r0 = threadIdx.x / (TL / 2);
+      const unsigned so = (unsigned)ko * (unsigned)a.outer_stride + (unsigned)kx0 + r0 * (unsigned)a.line_stride + 2 * ch;
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int i = 0; i < H / RPI; ++i) {
+          const int n = r0 + RPI * i;
+          cpa_zfill<16>(xst + (c * H + n) * TL + 2 * ch,
+                        a.spec + (so + (unsigned)c * (unsigned)a.comp_stride + (unsigned)(RPI * i) * (unsigned)a.line_stride),
+                        n < a.n_valid);
+        }
+    } else {
+      const int ko0 = (tile - ntm) * TL;
+      for (int q = threadIdx.x; q < 3 * H * TL; q += NT) {
+        const int row = q / TL, l = q % TL;
+        const int c = row / H, n = row % H;
+        const bool v = n < a.n_valid && ko0 + l < a.p_outer;
+        const int ko = v ? ko0 + l : 0;
+        cpa_zfill<8>(xst + row * TL + l,
+                     a.spec + (size_t)ko * a.outer_stride + (a.xc - 1) + (size_t)c * a.comp_stride + (size_t)n * a.line_stride, v);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  auto issue_k = [&](int tile) {
+    if (tile < ntm) {
+      const int ko = tile_ko(tile);
+      const int kom = (a.p_outer > 1 && 2 * ko > a.p_outer) ? a.p_outer - ko : ko;
+      const int kx0 = (tile - (tile / a.ntile_main) * a.ntile_main) * TL;
+      const unsigned kb = (unsigned)kom * (unsigned)a.k_outer_stride + (unsigned)kx0;
+      for (int q = threadIdx.x; q < 6 * (H + 1) * (TL / 4); q += NT) {
+        const int row = q / (TL / 4), ch = q % (TL / 4);
+        const int c = row / (H + 1), pm = row - c * (H + 1);
+        const unsigned sa = (unsigned)__cvta_generic_to_shared(kst + row * TL + 4 * ch);
+        const float* g = a.khat + (kb + (unsigned)c * (unsigned)a.k_comp_stride + (unsigned)pm * (unsigned)a.k_inner_stride + 4 * ch);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(g) : "memory");
+      }
+    } else {
+      const int ko0 = (tile - ntm) * TL;
+      for (int q = threadIdx.x; q < 6 * (H + 1) * TL; q += NT) {
+        const int row = q / TL, l = q % TL;
+        const int c = row / (H + 1), pm = row - c * (H + 1);
+        const bool v = ko0 + l < a.p_outer;
+        const int ko = v ? ko0 + l : 0;
+        const int kom = (a.p_outer > 1 && 2 * ko > a.p_outer) ? a.p_outer - ko : ko;
+        const unsigned sa = (unsigned)__cvta_generic_to_shared(kst + row * TL + l);
+        const float* g = a.khat + (size_t)kom * a.k_outer_stride + (a.xc - 1) + (size_t)c * a.k_comp_stride + (size_t)pm * a.k_inner_stride;
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(g) : "memory");
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  int tile = blockIdx.x;
+  if (tile < nt) { issue_x(tile); issue_k(tile); }
+  for (; tile < nt; tile += gridDim.x) {
+    const int nxt = tile + gridDim.x;
+    int kx, ko;
+    bool ok = true;
+    if (tile < ntm) {
+      ko = tile_ko(tile);
+      kx = (tile - (tile / a.ntile_main) * a.ntile_main) * TL + kxl;
+      ok = kx < a.xc_main;
+    } else {
+      kx = a.xc - 1; ko = (tile - ntm) * TL + kxl; ok = ko < a.p_outer;
+      if (!ok) ko = 0;
+    }
+    const int so = (a.p_outer > 1 && 2 * ko > a.p_outer) ? 1 : 0;
+    asm volatile("cp.async.wait_group 1;" ::: "memory");  // the spectrum stage (the kernel stage may still fly)
+    __syncthreads();  // tile has landed for every thread; exchange tiles of the previous tile are free
+    float2 X[3][R];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+      for (int u = 0; u < R; ++u) X[c][u] = cmul(xst[(c * H + j + R * u) * TL + kxl], twp[u]);
+      Dft<R, -1>::run(X[c]);
+      float2* t = sm + (c * 2 + h) * EXT + kxl;
+      t[(0 * R + j) * TL] = X[c][0];
+#pragma unroll
+      for (int q = 1; q < R; ++q) t[(q * R + j) * TL] = cmul(X[c][q], tws[q]);
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");  // kernel stage of this tile
+    __syncthreads();
+    if (nxt < nt) issue_x(nxt);  // the spectrum stage has been read by everyone
+    else asm volatile("cp.async.commit_group;" ::: "memory");
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float2* t = sm + (c * 2 + h) * EXT + kxl;
+#pragma unroll
+      for (int q = 0; q < R; ++q) X[c][q] = t[(j * R + q) * TL];
+      Dft<R, -1>::run(X[c]);
+    }
+    // B^_i = sum_j K^_ij M^_j ; K^ real, octant + parity (sign bit flips)
+    const unsigned mo3 = (so & (a.odd_outer >> 3)) << 31, mo4 = (so & (a.odd_outer >> 4)) << 31, mo5 = (so & (a.odd_outer >> 5)) << 31;
+    const unsigned mi3 = ((a.odd_inner >> 3) & 1u) << 31, mi4 = ((a.odd_inner >> 4) & 1u) << 31, mi5 = ((a.odd_inner >> 5) & 1u) << 31;
+#pragma unroll
+    for (int b = 0; b < R; ++b) {
+      const int kz = 2 * (j + R * b) + h;
+      const bool mir = 2 * kz > P;
+      const int pm = mir ? P - kz : kz;
+      const float* kp = kst + pm * TL + kxl;
+      const float k0 = kp[0 * (H + 1) * TL], k1 = kp[1 * (H + 1) * TL], k2 = kp[2 * (H + 1) * TL];
+      const float k3 = __uint_as_float(__float_as_uint(kp[3 * (H + 1) * TL]) ^ mo3 ^ (mir ? mi3 : 0u));
+      const float k4 = __uint_as_float(__float_as_uint(kp[4 * (H + 1) * TL]) ^ mo4 ^ (mir ? mi4 : 0u));
+      const float k5 = __uint_as_float(__float_as_uint(kp[5 * (H + 1) * TL]) ^ mo5 ^ (mir ? mi5 : 0u));
+      const float2 mx = X[0][b], my = X[1][b], mz = X[2][b];
+      X[0][b] = make_float2(fmaf(k0, mx.x, fmaf(k3, my.x, k4 * mz.x)), fmaf(k0, mx.y, fmaf(k3, my.y, k4 * mz.y)));
+      X[1][b] = make_float2(fmaf(k3, mx.x, fmaf(k1, my.x, k5 * mz.x)), fmaf(k3, mx.y, fmaf(k1, my.y, k5 * mz.y)));
+      X[2][b] = make_float2(fmaf(k4, mx.x, fmaf(k5, my.x, k2 * mz.x)), fmaf(k4, mx.y, fmaf(k5, my.y, k2 * mz.y)));
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      Dft<R, +1>::run(X[c]);
+      float2* t = sm + (c * 2 + h) * EXT + kxl;
+      t[(j * R + 0) * TL] = X[c][0];
+#pragma unroll
+      for (int q = 1; q < R; ++q) t[(j * R + q) * TL] = cmulc(X[c][q], tws[q]);
+    }
+    __syncthreads();
+    if (nxt < nt) issue_k(nxt);  // every thread is past the multiply: the kernel stage is free
+    else asm volatile("cp.async.commit_group;" ::: "memory");
+    const unsigned soff = (unsigned)ko * (unsigned)a.outer_stride + (unsigned)kx;
+    const unsigned sls = (unsigned)a.line_stride, scs = (unsigned)a.comp_stride;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float2* t = sm + (c * 2 + h) * EXT + kxl;
+#pragma unroll
+      for (int q = 0; q < R; ++q) X[c][q] = t[(q * R + j) * TL];
+      Dft<R, +1>::run(X[c]);
+#pragma unroll
+      for (int b = 0; b < R; ++b) X[c][b] = cmulc(X[c][b], twp[b]);
+#pragma unroll
+      for (int bb = 0; bb < R / 2; ++bb) {
+        const float2 mine = h ? X[c][bb + R / 2] : X[c][bb];
+        const float2 send = h ? X[c][bb] : X[c][bb + R / 2];
+        float2 recv;
+        recv.x = __shfl_xor_sync(0xffffffffu, send.x, TL);
+        recv.y = __shfl_xor_sync(0xffffffffu, send.y, TL);
+        const int n = j + R * (h ? bb + R / 2 : bb);
+        if (ok && n < a.n_valid) a.spec[soff + c * scs + (unsigned)n * sls] = cadd(mine, recv);
+      }
+    }
+  }
+}
+
 struct MidColArgs {
   const float2* in;
   float2* out;
@@ -862,8 +1040,11 @@ __global__ void __launch_bounds__(2 * R * TILE, 1) k_mid_colp(MidColArgs a) {
 // (lane = column + 8 h + 16 (j & 1)), the rows of the next tile stream into shared memory with
 // cp.async while the current tile is transformed; the halves of the inverse meet by shuffle.
 // Small CTAs (16 R threads, 65-97 KB) so that three (forward) or two (inverse) of them share an SM.
+#ifndef MMX_MIDP_TW_REGS
+#define MMX_MIDP_TW_REGS 1   // stage twiddles of a thread live in registers for the whole kernel
+#endif
 #ifndef MMX_MIDP_MINB_F
-#define MMX_MIDP_MINB_F 3
+#define MMX_MIDP_MINB_F 2   // (2 CTAs of 128 registers beat 3 of 80 once the twiddles are register-resident)
 #endif
 #ifndef MMX_MIDP_MINB_I
 #define MMX_MIDP_MINB_I 2
@@ -884,6 +1065,21 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
   const int ntm = a.ntile_main * a.nslab;
   const int nt = ntm + (a.nyq ? (a.nslab + TL - 1) / TL : 0);
   float2* ex = exb + h * EXT + kxl;
+#if MMX_MIDP_TW_REGS
+  // stage twiddles w_H^(j q) of this thread, loaded once for all tiles
+  float2 tws[R];
+#pragma unroll
+  for (int q = 0; q < R; ++q) tws[q] = a.tw[2 * j * q];
+#define MMX_TWS(q) tws[q]
+  // forward pass: also the half twiddles w_P^(j + R u) (identity for the even half)
+  float2 twp[DIR < 0 ? R : 1];
+  if (DIR < 0) {
+#pragma unroll
+    for (int u = 0; u < R; ++u) twp[u] = h ? a.tw[j + R * u] : make_float2(1.f, 0.f);
+  }
+#else
+#define MMX_TWS(q) stw[2 * j * (q)]
+#endif
 
   auto issue = [&](int tile, int buf) {
     float2* dst = stage + (size_t)buf * ROWS * TL;
@@ -941,8 +1137,12 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
 #pragma unroll
       for (int u = 0; u < R; ++u) {
         const float2 x = xin[(j + R * u) * TL];
+#if MMX_MIDP_TW_REGS
+        v[u] = cmul(x, twp[u]);
+#else
         const float2 w = h ? stw[j + R * u] : make_float2(1.f, 0.f);
         v[u] = cmul(x, w);
+#endif
       }
     } else {
 #pragma unroll
@@ -951,7 +1151,7 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
     Dft<R, DIR>::run(v);
     ex[(0 * R + j) * TL] = v[0];
 #pragma unroll
-    for (int q = 1; q < R; ++q) ex[(q * R + j) * TL] = ctw<DIR>(v[q], stw[2 * j * q]);
+    for (int q = 1; q < R; ++q) ex[(q * R + j) * TL] = ctw<DIR>(v[q], MMX_TWS(q));
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < R; ++q) v[q] = ex[(j * R + q) * TL];
@@ -1006,7 +1206,9 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   InnerColArgs a;
   a.spec = L.spec; a.khat = d.khat; a.tw = L.tw; a.ctrl = w->d_ctrl; a.gated = 1;
   a.n_valid = L.n_valid; a.xc = d.xc; a.p_outer = L.p_outer;
-#if MMX_INNER_VARIANT == 2
+#if MMX_INNER_VARIANT == 3
+  constexpr int TL = 16;
+#elif MMX_INNER_VARIANT == 2
   constexpr int TL = MMX_INNER_TL;
 #elif MMX_INNER_VARIANT == 1
   constexpr int TL = 16;
@@ -1020,7 +1222,17 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   a.k_inner_stride = L.k_inner_stride; a.k_outer_stride = L.k_outer_stride; a.k_comp_stride = L.k_comp_stride;
   a.odd_inner = L.odd_inner; a.odd_outer = L.odd_outer;
   ProfScope ps(w, PK_INNER);
-#if MMX_INNER_VARIANT == 2
+#if MMX_INNER_VARIANT == 3
+  const size_t smem = sizeof(float2) * (6 + 3) * 64 * TL + sizeof(float) * 6 * 65 * TL;
+  if (int rc = set_smem_col(k_inner_q<8>, smem)) return rc;
+  const int nt = a.ntile_main * L.n_outer + (a.nyq ? (L.p_outer + TL - 1) / TL : 0);
+  int grid = 2 * w->sm_count;
+  if (grid > nt) grid = nt;
+  if (L.p_outer != L.n_outer) return mmx_fail(MMX_EINVAL, "inner column pass: outer extent mismatch");
+  if (3 * L.comp_stride >= (1ull << 31) || 6 * L.k_comp_stride >= (1ull << 31))
+    return mmx_fail(MMX_EINVAL, "inner column pass: spectra exceed the 32-bit element offsets of this kernel");
+  k_inner_q<8><<<grid, 256, smem, w->stream>>>(a);
+#elif MMX_INNER_VARIANT == 2
   const size_t smem = sizeof(float2) * (6 * (64 * TL + (TL < 16 ? 8 : 0)) + 6 * 64 * TL);
   if (int rc = set_smem_col(k_inner_pipe<8, TL>, smem)) return rc;
   const int nt = a.ntile_main * L.n_outer + (a.nyq ? (L.p_outer + TL - 1) / TL : 0);
