@@ -28,21 +28,27 @@ namespace mmxreg {
 #ifndef MMX_PACKED_F32X2
 #define MMX_PACKED_F32X2 1
 #endif
-#if MMX_PACKED_F32X2
-MMX_DI float2 cadd(float2 a, float2 b) {
+#ifndef MMX_PACKED_R16
+#define MMX_PACKED_R16 MMX_PACKED_F32X2   // the radix-16 butterflies of the y passes run better on scalar adds
+#endif
+MMX_DI float2 cadd_pk(float2 a, float2 b) {
   unsigned long long ua = *reinterpret_cast<unsigned long long*>(&a), ub = *reinterpret_cast<unsigned long long*>(&b), ud;
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(ud) : "l"(ua), "l"(ub));
   return *reinterpret_cast<float2*>(&ud);
 }
-MMX_DI float2 csub(float2 a, float2 b) {
+MMX_DI float2 csub_pk(float2 a, float2 b) {
   unsigned long long ua = *reinterpret_cast<unsigned long long*>(&a), ub = *reinterpret_cast<unsigned long long*>(&b), ud;
   asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(ud) : "l"(ua), "l"(ub));
   return *reinterpret_cast<float2*>(&ud);
 }
-#else
-MMX_DI float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-MMX_DI float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-#endif
+MMX_DI float2 cadd_sc(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+MMX_DI float2 csub_sc(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+template <bool PK>
+MMX_DI float2 caddt(float2 a, float2 b) { return PK ? cadd_pk(a, b) : cadd_sc(a, b); }
+template <bool PK>
+MMX_DI float2 csubt(float2 a, float2 b) { return PK ? csub_pk(a, b) : csub_sc(a, b); }
+MMX_DI float2 cadd(float2 a, float2 b) { return caddt<MMX_PACKED_F32X2 != 0>(a, b); }
+MMX_DI float2 csub(float2 a, float2 b) { return csubt<MMX_PACKED_F32X2 != 0>(a, b); }
 MMX_DI float2 cmul(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
@@ -77,13 +83,13 @@ MMX_DI float2 csub_i(float2 b, float2 d) {
   return DIR < 0 ? make_float2(b.x - d.y, b.y + d.x) : make_float2(b.x + d.y, b.y - d.x);
 }
 
-template <int DIR>
+template <int DIR, bool PK = (MMX_PACKED_F32X2 != 0)>
 MMX_DI void dft4(float2& x0, float2& x1, float2& x2, float2& x3) {
-  const float2 a = cadd(x0, x2), b = csub(x0, x2);
-  const float2 c = cadd(x1, x3), d = csub(x1, x3);
-  x0 = cadd(a, c);
+  const float2 a = caddt<PK>(x0, x2), b = csubt<PK>(x0, x2);
+  const float2 c = caddt<PK>(x1, x3), d = csubt<PK>(x1, x3);
+  x0 = caddt<PK>(a, c);
   x1 = cadd_i<DIR>(b, d);
-  x2 = csub(a, c);
+  x2 = csubt<PK>(a, c);
   x3 = csub_i<DIR>(b, d);
 }
 
@@ -124,7 +130,7 @@ struct Dft<16, DIR> {
 #pragma unroll
     for (int n2 = 0; n2 < 4; ++n2) {
       t[n2][0] = v[n2]; t[n2][1] = v[4 + n2]; t[n2][2] = v[8 + n2]; t[n2][3] = v[12 + n2];
-      dft4<DIR>(t[n2][0], t[n2][1], t[n2][2], t[n2][3]);
+      dft4<DIR, MMX_PACKED_R16 != 0>(t[n2][0], t[n2][1], t[n2][2], t[n2][3]);
     }
     // w16^(n2 k1)
     t[1][1] = rot<DIR>(t[1][1], c1, s1);
@@ -138,7 +144,7 @@ struct Dft<16, DIR> {
     t[3][3] = rot<DIR>(t[3][3], -c1, -s1);  // w16^9 = -w16^1
 #pragma unroll
     for (int k1 = 0; k1 < 4; ++k1) {
-      dft4<DIR>(t[0][k1], t[1][k1], t[2][k1], t[3][k1]);  // index k2 now lives in the first slot
+      dft4<DIR, MMX_PACKED_R16 != 0>(t[0][k1], t[1][k1], t[2][k1], t[3][k1]);  // index k2 now lives in the first slot
       v[k1] = t[0][k1]; v[k1 + 4] = t[1][k1]; v[k1 + 8] = t[2][k1]; v[k1 + 12] = t[3][k1];
     }
   }
