@@ -56,12 +56,16 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   const int nx = FULL ? XH : a.nx, S = FULL ? 1 : a.S;
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ float2 stw[XP];
+  // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
+  // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
+  __shared__ float2 stq[XR * (XR + 1)];
   if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   float* sin_ = reinterpret_cast<float*>(smraw + wid * xfwd_warp_bytes(S));
   float2* sex = reinterpret_cast<float2*>(sin_ + (size_t)S * 2 * XH);
   for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
+  for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
   const float* y = a.ctrl->sel ? a.yin[1] : a.yin[0];  // (no dynamic index into the parameter block)
   const int npair = (a.rows + 1) >> 1;
   const int nwarp = gridDim.x * XW;
@@ -110,7 +114,7 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
     float2* ex = sex + h * EXN;
     ex[padx(j)] = v[0];
 #pragma unroll
-    for (int q = 1; q < XR; ++q) ex[padx(q * XR + j)] = cmul(v[q], stw[2 * j * q]);
+    for (int q = 1; q < XR; ++q) ex[padx(q * XR + j)] = cmul(v[q], stq[j * (XR + 1) + q]);
     __syncwarp();
 #pragma unroll
     for (int q = 0; q < XR; ++q) v[q] = ex[padx(j * XR + q)];
@@ -145,11 +149,15 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   const int nx = FULL ? XH : a.nx;
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ float2 stw[XP];
+  // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
+  // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
+  __shared__ float2 stq[XR * (XR + 1)];
   if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   XInvSmem& sm = reinterpret_cast<XInvSmem*>(smraw)[wid];
   for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
+  for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
   const int npair = (a.rows + 1) >> 1;
   const int nwarp = gridDim.x * XW;
   constexpr int CH = (XH + 1 + 1) / 2;  // 16-byte chunks covering 257 complex values
@@ -187,7 +195,7 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
     float2* ex = sm.ex + h * EXN;
     ex[padx(j)] = v[0];
 #pragma unroll
-    for (int q = 1; q < XR; ++q) ex[padx(q * XR + j)] = cmulc(v[q], stw[2 * j * q]);
+    for (int q = 1; q < XR; ++q) ex[padx(q * XR + j)] = cmulc(v[q], stq[j * (XR + 1) + q]);
     __syncwarp();
 #pragma unroll
     for (int q = 0; q < XR; ++q) v[q] = ex[padx(j * XR + q)];
