@@ -34,7 +34,7 @@ DT = {"c1": 1e-13, "c2": 2e-14, "c3": 5e-15, "c4": 1e-13, "c5": 5e-15}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
 # committed `ncu --set full` capture (profiles/, see the .md beside it); None until captured.
-NCU_TRAFFIC_BYTES = {"demag_inner": 339184896 + 170884096}  # profiles/ncu_r1_kernels.md (k_inner_pipe<8,16>)
+NCU_TRAFFIC_BYTES = {"demag_inner": 339593984 + 166750208}  # profiles/ncu_r1_kernels.md (k_inner_q<8>)
 
 
 def measured_peaks():

@@ -271,8 +271,11 @@ __device__ __forceinline__ void stq(float* p, size_t N, size_t i, const Q3& q) {
 #endif
 // NP = n_prev, the number of earlier k_j of the RK combination; MODE bit 0: form the next stage
 // state, bit 1: form the embedded error
+#ifndef MMX_L4_BLOCK
+#define MMX_L4_BLOCK 256
+#endif
 template <int S, int NP, int MODE>
-__global__ void __launch_bounds__(256, MMX_L4_MINB) k_local4(LocalArgs a) {
+__global__ void __launch_bounds__(MMX_L4_BLOCK, MMX_L4_MINB) k_local4(LocalArgs a) {
   // thread-private landing slots for the streamed inputs (B_demag, y0, k_j): cp.async puts them
   // in flight at the top of the kernel without holding registers; slot a of thread t is
   // lsm[a * 256 + t] (16 B per lane: conflict-free)
@@ -285,14 +288,14 @@ __global__ void __launch_bounds__(256, MMX_L4_MINB) k_local4(LocalArgs a) {
   auto stage3 = [&](int slot, const float* p, size_t idx) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      const unsigned sa = (unsigned)__cvta_generic_to_shared(&lsm[(slot + c) * 256 + threadIdx.x]);
+      const unsigned sa = (unsigned)__cvta_generic_to_shared(&lsm[(slot + c) * MMX_L4_BLOCK + threadIdx.x]);
       asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(p + (size_t)c * N + idx) : "memory");
     }
   };
   auto take3 = [&](int slot) -> Q3 {
-    const float4 x = lsm[(slot + 0) * 256 + threadIdx.x];
-    const float4 y = lsm[(slot + 1) * 256 + threadIdx.x];
-    const float4 z = lsm[(slot + 2) * 256 + threadIdx.x];
+    const float4 x = lsm[(slot + 0) * MMX_L4_BLOCK + threadIdx.x];
+    const float4 y = lsm[(slot + 1) * MMX_L4_BLOCK + threadIdx.x];
+    const float4 z = lsm[(slot + 2) * MMX_L4_BLOCK + threadIdx.x];
     Q3 q;
     q.c[0] = v3(x.x, y.x, z.x); q.c[1] = v3(x.y, y.y, z.y); q.c[2] = v3(x.z, y.z, z.z); q.c[3] = v3(x.w, y.w, z.w);
     return q;
@@ -642,14 +645,14 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   bool uniform = !reg && (w->grid[0] % 4) == 0;
   for (int s = 0; s < w->S && uniform; ++s) uniform = w->mats[(size_t)s * w->nreg].Ms > 0;
   if (uniform) {
-    const unsigned b4 = (unsigned)((N / 4 + 255) / 256);
+    const unsigned b4 = (unsigned)((N / 4 + MMX_L4_BLOCK - 1) / MMX_L4_BLOCK);
     const int mode = (a.ynext[0] ? 1 : 0) | (a.do_err ? 2 : 0);
 #define MMX_L4_GO(S_, NP_, M_)                                                             \
   {                                                                                        \
-    const size_t sm_ = sizeof(float4) * 256 * (6 + 3 * (NP_));                             \
+    const size_t sm_ = sizeof(float4) * MMX_L4_BLOCK * (6 + 3 * (NP_));                            \
     if (sm_ > 32 * 1024)                                                                   \
       MMX_CUDA(cudaFuncSetAttribute(k_local4<S_, NP_, M_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_)); \
-    k_local4<S_, NP_, M_><<<b4, 256, sm_, w->stream>>>(a);                                 \
+    k_local4<S_, NP_, M_><<<b4, MMX_L4_BLOCK, sm_, w->stream>>>(a);                                \
   }
 #define MMX_L4(S_, NP_)                                                    \
   case NP_:                                                                \
