@@ -672,7 +672,6 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_q(InnerColArgs a) {
   float2* sm = reinterpret_cast<float2*>(smraw);             // exchange [3][2][H][TL]
   float2* xst = sm + 6 * EXT;                                // spectrum stage [3][H][TL]
   float* kst = reinterpret_cast<float*>(xst + 3 * H * TL);   // kernel stage [6][H+1][TL]
-  if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
   const int kxl = lane & 15, h = lane >> 4;
   const int ntm = a.ntile_main * a.p_outer;
@@ -684,6 +683,10 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_q(InnerColArgs a) {
     tws[q] = a.tw[2 * j * q];
     twp[q] = h ? a.tw[j + R * q] : make_float2(1.f, 0.f);
   }
+
+  pdl_wait();      // the twiddle loads above do not depend on the previous kernel
+  pdl_trigger();   // persistent kernel: the next kernel's CTAs take over as ours exit
+  if (a.gated && !a.ctrl->active) return;
 
   auto tile_ko = [&](int tile) -> int {
     const int yy = tile / a.ntile_main;
@@ -1059,7 +1062,6 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
   float2* exb = reinterpret_cast<float2*>(smraw);   // [2][EXT]
   float2* stage = exb + 2 * EXT;                     // [2][ROWS][TL]
   __shared__ float2 stw[P];
-  if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int kxl = lane & 7, h = (lane >> 3) & 1, j = 2 * wid + (lane >> 4);
   for (int q = threadIdx.x; q < P; q += NT) stw[q] = a.tw[q];
@@ -1081,6 +1083,10 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
 #else
 #define MMX_TWS(q) stw[2 * j * (q)]
 #endif
+
+  pdl_wait();      // the twiddle loads above do not depend on the previous kernel
+  pdl_trigger();   // persistent kernel: the next kernel's CTAs take over as ours exit
+  if (a.gated && !a.ctrl->active) return;
 
   auto issue = [&](int tile, int buf) {
     float2* dst = stage + (size_t)buf * ROWS * TL;
@@ -1227,12 +1233,12 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   const size_t smem = sizeof(float2) * (6 + 3) * 64 * TL + sizeof(float) * 6 * 65 * TL;
   if (int rc = set_smem_col(k_inner_q<8>, smem)) return rc;
   const int nt = a.ntile_main * L.n_outer + (a.nyq ? (L.p_outer + TL - 1) / TL : 0);
-  int grid = 2 * w->sm_count;
+  int grid = mmx_persistent_grid(k_inner_q<8>, 256, smem, w->sm_count, 2);
   if (grid > nt) grid = nt;
   if (L.p_outer != L.n_outer) return mmx_fail(MMX_EINVAL, "inner column pass: outer extent mismatch");
   if (3 * L.comp_stride >= (1ull << 31) || 6 * L.k_comp_stride >= (1ull << 31))
     return mmx_fail(MMX_EINVAL, "inner column pass: spectra exceed the 32-bit element offsets of this kernel");
-  k_inner_q<8><<<grid, 256, smem, w->stream>>>(a);
+  MMX_CUDA(mmx_launch(k_inner_q<8>, grid, 256, smem, w->stream, a));
 #elif MMX_INNER_VARIANT == 2
   const size_t smem = sizeof(float2) * (6 * (64 * TL + (TL < 16 ? 8 : 0)) + 6 * 64 * TL);
   if (int rc = set_smem_col(k_inner_pipe<8, TL>, smem)) return rc;
@@ -1289,12 +1295,12 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
     const size_t sm = sizeof(float2) * (2 * (R * R * TL + 8) + 2 * (dir < 0 ? R * R : 2 * R * R) * TL);
     if (dir < 0) {
       if (int rc = set_smem_col(k_mid_pipe<16, -1>, sm)) return rc;
-      int grid = MMX_MIDP_MINB_F * w->sm_count;
-      k_mid_pipe<16, -1><<<grid < nt ? grid : nt, 16 * 16, sm, w->stream>>>(b);
+      int grid = mmx_persistent_grid(k_mid_pipe<16, -1>, 16 * 16, sm, w->sm_count, MMX_MIDP_MINB_F);
+      MMX_CUDA(mmx_launch(k_mid_pipe<16, -1>, grid < nt ? grid : nt, 16 * 16, sm, w->stream, b));
     } else {
       if (int rc = set_smem_col(k_mid_pipe<16, +1>, sm)) return rc;
-      int grid = MMX_MIDP_MINB_I * w->sm_count;
-      k_mid_pipe<16, +1><<<grid < nt ? grid : nt, 16 * 16, sm, w->stream>>>(b);
+      int grid = mmx_persistent_grid(k_mid_pipe<16, +1>, 16 * 16, sm, w->sm_count, MMX_MIDP_MINB_I);
+      MMX_CUDA(mmx_launch(k_mid_pipe<16, +1>, grid < nt ? grid : nt, 16 * 16, sm, w->stream, b));
     }
     MMX_CUDA(cudaGetLastError());
     return MMX_OK;

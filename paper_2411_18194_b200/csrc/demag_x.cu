@@ -59,13 +59,15 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
   // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
   __shared__ float2 stq[XR * (XR + 1)];
-  if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   float* sin_ = reinterpret_cast<float*>(smraw + wid * xfwd_warp_bytes(S));
   float2* sex = reinterpret_cast<float2*>(sin_ + (size_t)S * 2 * XH);
   for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
   for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
+  pdl_wait();      // everything above is independent of the previous kernel
+  pdl_trigger();   // persistent kernel: the next kernel's CTAs may take over the SMs as ours exit
+  if (a.gated && !a.ctrl->active) return;
   const float* y = a.ctrl->sel ? a.yin[1] : a.yin[0];  // (no dynamic index into the parameter block)
   const int npair = (a.rows + 1) >> 1;
   const int nwarp = gridDim.x * XW;
@@ -152,12 +154,14 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
   // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
   __shared__ float2 stq[XR * (XR + 1)];
-  if (a.gated && !a.ctrl->active) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   XInvSmem& sm = reinterpret_cast<XInvSmem*>(smraw)[wid];
   for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
   for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
+  pdl_wait();      // everything above is independent of the previous kernel
+  pdl_trigger();   // persistent kernel: the next kernel's CTAs may take over the SMs as ours exit
+  if (a.gated && !a.ctrl->active) return;
   const int npair = (a.rows + 1) >> 1;
   const int nwarp = gridDim.x * XW;
   constexpr int CH = (XH + 1 + 1) / 2;  // 16-byte chunks covering 257 complex values
@@ -248,28 +252,42 @@ int mmx_x_warp_launch(mmx_world* w, int dir, const float* const yin[2], float* b
   a.yin[0] = yin ? yin[0] : nullptr; a.yin[1] = yin ? yin[1] : nullptr;
   a.ctrl = w->d_ctrl; a.tw = d.tw[0]; a.spec = d.spec1; a.bout = bout;
   const int npair = (a.rows + 1) / 2;
-  int blocks = (dir < 0 ? 4 : 3) * w->sm_count;
-  if (blocks * XW > npair) blocks = (npair + XW - 1) / XW;
   const bool full = d.nx == XH && (a.rows & 1) == 0 && w->S == 1;
+  int blocks;
+  {
+    const size_t smem = dir < 0 ? xfwd_warp_bytes(a.S) * XW : sizeof(XInvSmem) * XW;
+    if (dir < 0) {
+      MMX_CUDA(cudaFuncSetAttribute(k_x_fwd_w<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      MMX_CUDA(cudaFuncSetAttribute(k_x_fwd_w<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      blocks = full ? mmx_persistent_grid(k_x_fwd_w<true>, 32 * XW, smem, w->sm_count, 4)
+                    : mmx_persistent_grid(k_x_fwd_w<false>, 32 * XW, smem, w->sm_count, 4);
+    } else {
+      MMX_CUDA(cudaFuncSetAttribute(k_x_inv_w<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      MMX_CUDA(cudaFuncSetAttribute(k_x_inv_w<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      blocks = full ? mmx_persistent_grid(k_x_inv_w<true>, 32 * XW, smem, w->sm_count, 3)
+                    : mmx_persistent_grid(k_x_inv_w<false>, 32 * XW, smem, w->sm_count, 3);
+    }
+  }
+  if (blocks * XW > npair) blocks = (npair + XW - 1) / XW;
   if (dir < 0) {
     const size_t smem = xfwd_warp_bytes(a.S) * XW;
     ProfScope ps(w, PK_X_FWD);
     if (full) {
       MMX_CUDA(cudaFuncSetAttribute(k_x_fwd_w<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k_x_fwd_w<true><<<blocks, 32 * XW, smem, w->stream>>>(a);
+      MMX_CUDA(mmx_launch(k_x_fwd_w<true>, blocks, 32 * XW, smem, w->stream, a));
     } else {
       MMX_CUDA(cudaFuncSetAttribute(k_x_fwd_w<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k_x_fwd_w<false><<<blocks, 32 * XW, smem, w->stream>>>(a);
+      MMX_CUDA(mmx_launch(k_x_fwd_w<false>, blocks, 32 * XW, smem, w->stream, a));
     }
   } else {
     const size_t smem = sizeof(XInvSmem) * XW;
     ProfScope ps(w, PK_X_INV);
     if (full) {
       MMX_CUDA(cudaFuncSetAttribute(k_x_inv_w<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k_x_inv_w<true><<<blocks, 32 * XW, smem, w->stream>>>(a);
+      MMX_CUDA(mmx_launch(k_x_inv_w<true>, blocks, 32 * XW, smem, w->stream, a));
     } else {
       MMX_CUDA(cudaFuncSetAttribute(k_x_inv_w<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k_x_inv_w<false><<<blocks, 32 * XW, smem, w->stream>>>(a);
+      MMX_CUDA(mmx_launch(k_x_inv_w<false>, blocks, 32 * XW, smem, w->stream, a));
     }
   }
   MMX_CUDA(cudaGetLastError());

@@ -281,6 +281,7 @@ __global__ void __launch_bounds__(MMX_L4_BLOCK, MMX_L4_MINB) k_local4(LocalArgs 
   // lsm[a * 256 + t] (16 B per lane: conflict-free)
   extern __shared__ float4 lsm[];
   MmxCtrl* ctrl = a.ctrl;
+  pdl_wait();  // (multi-wave kernel: no early trigger, its own pending CTAs need the SM slots)
   if (!ctrl->active) return;
   const int sel = ctrl->sel;
   const size_t N = (size_t)a.nx * a.ny * a.nz;
@@ -531,6 +532,7 @@ __global__ void __launch_bounds__(MMX_L4_BLOCK, MMX_L4_MINB) k_local4(LocalArgs 
 __global__ void __launch_bounds__(256) k_combine1(const float* y0a, const float* y0b, const float* k1a,
                                                   const float* k1b, float* yna, float* ynb, int row, int S,
                                                   int nvec, size_t N, MmxCtrl* ctrl) {
+  pdl_wait();
   if (!ctrl->active) return;
   const int sel = ctrl->sel;
   const float* y0 = sel ? y0b : y0a;
@@ -555,6 +557,7 @@ __global__ void __launch_bounds__(256) k_combine1(const float* y0a, const float*
 // mode 2: re-arm (active = 1) after a stepping call
 // mode 3: first step size from max torque: dt = 0.01 / max|tau| (only when dt <= 0)
 __global__ void k_controller(MmxCtrl* c, MmxTableau tab, int mode) {
+  pdl_wait();
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   if (mode == 2) { c->active = 1; return; }
   if (mode == 3) {
@@ -652,7 +655,7 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
     const size_t sm_ = sizeof(float4) * MMX_L4_BLOCK * (6 + 3 * (NP_));                            \
     if (sm_ > 32 * 1024)                                                                   \
       MMX_CUDA(cudaFuncSetAttribute(k_local4<S_, NP_, M_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_)); \
-    k_local4<S_, NP_, M_><<<b4, MMX_L4_BLOCK, sm_, w->stream>>>(a);                                \
+    MMX_CUDA(mmx_launch(k_local4<S_, NP_, M_>, b4, MMX_L4_BLOCK, sm_, w->stream, a));                                \
   }
 #define MMX_L4(S_, NP_)                                                    \
   case NP_:                                                                \
@@ -680,8 +683,8 @@ int mmx_combine_launch(mmx_world* w, const float* const y0[2], const float* cons
                        float* const ynext[2], int row) {
   const unsigned blocks = (unsigned)((w->N + 255) / 256);
   ProfScope ps(w, PK_COMBINE);
-  k_combine1<<<blocks, 256, 0, w->stream>>>(y0[0], y0[1], k1[0], k1[1], ynext[0], ynext[1], row, w->S,
-                                            w->nvec, w->N, w->d_ctrl);
+  MMX_CUDA(mmx_launch(k_combine1, blocks, 256, 0, w->stream, y0[0], y0[1], k1[0], k1[1], ynext[0], ynext[1], row,
+                      w->S, w->nvec, w->N, w->d_ctrl));
   w->launches++;
   MMX_CUDA(cudaGetLastError());
   return MMX_OK;
@@ -689,7 +692,7 @@ int mmx_combine_launch(mmx_world* w, const float* const y0[2], const float* cons
 
 int mmx_controller_launch(mmx_world* w, const MmxTableau& tab, int mode) {
   ProfScope ps(w, PK_CTRL);
-  k_controller<<<1, 32, 0, w->stream>>>(w->d_ctrl, tab, mode);
+  MMX_CUDA(mmx_launch(k_controller, 1, 32, 0, w->stream, w->d_ctrl, tab, mode));
   w->launches++;
   MMX_CUDA(cudaGetLastError());
   return MMX_OK;
