@@ -55,7 +55,7 @@ template <bool FULL>
 __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   const int nx = FULL ? XH : a.nx, S = FULL ? 1 : a.S;
   extern __shared__ __align__(16) unsigned char smraw[];
-  __shared__ float2 stw[XP];
+  __shared__ float2 stw[XH];  // w_P^n for n < P/2 only (the half twiddles of the pruned input)
   // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
   // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
   __shared__ float2 stq[XR * (XR + 1)];
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   float* sin_ = reinterpret_cast<float*>(smraw + wid * xfwd_warp_bytes(S));
   float2* sex = reinterpret_cast<float2*>(sin_ + (size_t)S * 2 * XH);
-  for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
+  for (int q = threadIdx.x; q < XH; q += 32 * XW) stw[q] = a.tw[q];
   for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
   pdl_wait();      // everything above is independent of the previous kernel
   pdl_trigger();   // persistent kernel: the next kernel's CTAs may take over the SMs as ours exit
@@ -150,14 +150,14 @@ template <bool FULL>
 __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   const int nx = FULL ? XH : a.nx;
   extern __shared__ __align__(16) unsigned char smraw[];
-  __shared__ float2 stw[XP];
+  __shared__ float2 stw[XH];  // conj(w_P^n) for the first P/2 outputs only
   // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
   // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
   __shared__ float2 stq[XR * (XR + 1)];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   XInvSmem& sm = reinterpret_cast<XInvSmem*>(smraw)[wid];
-  for (int q = threadIdx.x; q < XP; q += 32 * XW) stw[q] = a.tw[q];
+  for (int q = threadIdx.x; q < XH; q += 32 * XW) stw[q] = a.tw[q];
   for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
   pdl_wait();      // everything above is independent of the previous kernel
   pdl_trigger();   // persistent kernel: the next kernel's CTAs may take over the SMs as ours exit
