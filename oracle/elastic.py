@@ -90,6 +90,14 @@ def stress(eps, C11, C12, C44):
                 xy=2 * C44 * eps["xy"], xz=2 * C44 * eps["xz"], yz=2 * C44 * eps["yz"])
 
 
+def viscous_stress(v, beta, C11, C12, C44, cell, pbc):
+    """"viscous damping, where an extra term, proportional to the strain rate, is added to
+    the total stress tensor"; Table 1 names its coefficient "stiffness coefficient of the
+    Rayleigh damping", a time (0.1 ps).  Reading S31: stiffness-proportional Rayleigh
+    damping, sigma_visc = beta C : eps_dot with eps_dot = sym grad v (same gradient operator)."""
+    return {k: beta * val for k, val in stress(strain(v, cell, pbc), C11, C12, C44).items()}
+
+
 def div_axis(s, axis, h, periodic, face_lo, face_hi):
     """d s / d x_axis with the face values of s on the two open faces of that axis."""
     n = s.shape[s.ndim - 1 - axis]

@@ -135,9 +135,13 @@ class World:
         amp = tr["amp"] * np.sin(2 * np.pi * tr["freq"] * t)
         return {tr["face"]: amp * np.asarray(tr["vec"], float)}
 
-    def acceleration(self, m, u, t):
+    def acceleration(self, m, u, t, v=None):
         e = self.elastic
         sig = el.stress(el.strain(u, self.cell, self.pbc), e["C11"], e["C12"], e["C44"])
+        beta = e.get("beta", 0.0)
+        if beta and v is not None:  # viscous (Rayleigh, stiffness-proportional) term
+            sv = el.viscous_stress(v, beta, e["C11"], e["C12"], e["C44"], self.cell, self.pbc)
+            sig = {k: sig[k] + sv[k] for k in sig}
         f = el.elastic_force(sig, self.cell, self.pbc, self.tractions(t))
         for s in range(self.S):
             f = f + el.magnetoelastic_force(m[s], self.p[s]["B1"], self.p[s]["B2"], self.cell, self.pbc)
@@ -162,7 +166,7 @@ class World:
         bd = self.demag_field(m) if self.use_demag else None
         k = [self.torque(s, m, u, T_ALL, bd) for s in range(self.S)]
         if self.elastic is not None:
-            k += [y[self.S + 1].copy(), self.acceleration(m, u, t)]
+            k += [y[self.S + 1].copy(), self.acceleration(m, u, t, y[self.S + 1])]
         return k
 
     def project(self, y):

@@ -122,6 +122,50 @@ def test_P15_paper_pulse_speed_and_strain():
     assert abs(amp - t0 / (2 * C44)) < 0.02 * t0 / (2 * C44)
 
 
+def test_P20_rayleigh_damping_ratio_of_the_paper():
+    """Table 1: Rayleigh stiffness coefficient 0.1 ps, "chosen to yield a damping ratio of
+    about 5% for shear waves with a wavelength of 24 nm" (C44 = 110 GPa, rho = 6853 kg/m^3).  A
+    periodic standing shear wave of that wavelength is integrated with the oracle; the decay of its
+    modal energy gives zeta.  Pins reading S31 (sigma_visc = beta C : strain rate): zeta = beta w0 / 2."""
+    want = _paper_numbers()
+    beta = want["rayleigh_beta_s"][0]
+    n, h = 48, 3e-9                      # wavelength 24 nm = 8 cells
+    C11, C12, C44, rho = 3.3e11, 0.6e11, 1.1e11, 6853.0
+    k = 2 * np.pi / 24e-9
+    x = np.arange(n) * h
+    u = np.zeros((3, 1, 1, n), np.float32)
+    u[2, 0, 0] = 1e-12 * np.sin(k * x)
+    spec = wl.WorldSpec(name="nio", grid=(n, 1, 1), cell=(h, h, h), pbc=(1, 0, 0), demag=False,
+                        mat=wl.make_mat(1, Ms=4.25e5), coupling=wl.default_coupling(),
+                        elastic=dict(C11=C11, C12=C12, C44=C44, rho=rho, beta=beta, traction=None),
+                        m=[np.tile(np.array([1, 0, 0], np.float32).reshape(3, 1, 1, 1), (1, 1, 1, n))],
+                        u=u, v=np.zeros_like(u))
+    w = World(spec)
+    keff = (8 * np.sin(k * h) - np.sin(2 * k * h)) / (6 * h)
+    w0 = keff * np.sqrt(C44 / rho)
+
+    def modal_energy():
+        a = 2.0 / n * (w.u[2, 0, 0] * np.sin(k * x)).sum()
+        adot = 2.0 / n * (w.v[2, 0, 0] * np.sin(k * x)).sum()
+        return w0 ** 2 * a ** 2 + adot ** 2
+
+    e0 = modal_energy()
+    dt = 5e-14                           # 121 steps per period: RK4 phase error ~ (w0 dt)^4 / 120 = 6e-8
+    nsteps = int(round(2 * 2 * np.pi / w0 / dt))
+    w.step_rk4(dt, nsteps)
+    zeta = -np.log(modal_energy() / e0) / (2 * w0 * nsteps * dt)
+    v, tol = want["damping_ratio_shear_24nm"]
+    assert abs(zeta - v) < tol * v, zeta                      # the paper's "about 5 %"
+    assert abs(zeta - 0.5 * beta * w0) < 0.01 * 0.5 * beta * w0, (zeta, 0.5 * beta * w0)
+    # and without the viscous term the same wave does not decay
+    spec.elastic["beta"] = 0.0
+    spec.u, spec.v = u, np.zeros_like(u)
+    w = World(spec)
+    e0 = modal_energy()
+    w.step_rk4(dt, nsteps)
+    assert abs(modal_energy() / e0 - 1) < 1e-6
+
+
 def test_P17_magnetoelastic_closed_forms():
     """Uniform strain, uniform m: Eq.9 closed form and f_mel = 0; f_mel = div sigma_mel with
     sigma_mel,ii = B1 m_i^2, sigma_mel,ij = B2 m_i m_j for a smooth texture."""
