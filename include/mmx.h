@@ -109,6 +109,9 @@ typedef struct mmx_elastic {
   double traction_vec[3]; /* direction of t in sigma.n = t                             */
   double traction_amp;    /* Pa                                                        */
   double traction_freq;   /* Hz; t(t) = amp * sin(2 pi freq t) * vec                   */
+  double rayleigh_beta;   /* s; viscous term beta C : strain rate added to the stress  */
+                          /* (Table 1 "stiffness coefficient of the Rayleigh   */
+                          /* damping", 0.1 ps for NiO); 0 = undamped                   */
 } mmx_elastic;
 
 typedef struct mmx_rk_opts {

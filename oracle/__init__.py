@@ -17,7 +17,7 @@ Pin status (see tests/test_oracle_*.py and DESIGN.md section "Oracle pins"):
   sublattice exchange ..... pinned (P10, P12)
   LLG torque, integrators . pinned (P7, P8, P9, P14)
   Zhang-Li torque ......... pinned (P13: Gilbert-form identity, rigid translation at -u)
-  elastic / magnetoelastic  pinned (P15 paper numbers, P16 patch test, P17)
+  elastic / magnetoelastic  pinned (P15 paper numbers, P16 patch test, P17; viscous term P20 paper numbers)
   adaptive-step controller constants (S21), PBC image window (S13), which
   config switches c3 uses (S8, S14): parity unpinned -- definitions shared by
   both sides, stated in DESIGN.md.

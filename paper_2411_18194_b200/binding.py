@@ -46,7 +46,7 @@ class Coupling(C.Structure):
 class Elastic(C.Structure):
     _fields_ = [("C11", C.c_double), ("C12", C.c_double), ("C44", C.c_double), ("rho", C.c_double),
                 ("traction_face", C.c_int), ("traction_vec", C.c_double * 3),
-                ("traction_amp", C.c_double), ("traction_freq", C.c_double)]
+                ("traction_amp", C.c_double), ("traction_freq", C.c_double), ("rayleigh_beta", C.c_double)]
 
 
 class RkOpts(C.Structure):
@@ -229,6 +229,7 @@ class World:
             return
         s = Elastic()
         s.C11, s.C12, s.C44, s.rho = e["C11"], e["C12"], e["C44"], e["rho"]
+        s.rayleigh_beta = float(e.get("beta", 0.0))
         tr = e.get("traction")
         s.traction_face = -1
         if tr:

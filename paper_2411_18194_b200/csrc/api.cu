@@ -171,7 +171,12 @@ int upload_params(mmx_world* w) {
 
 int alloc_state(mmx_world* w) {
   const int nvec = w->S + (w->has_elastic ? 2 : 0);
-  if (w->Y[0] && nvec == w->nvec) return MMX_OK;
+  if (w->Y[0] && nvec == w->nvec) {
+    // the state keeps its shape; the viscous-damping strain buffer may still have been switched on
+    if (w->has_elastic && w->el.rayleigh_beta != 0.0 && !w->strain_f)
+      if (int rc = dev_alloc(w, &w->strain_f, 6 * w->N)) return rc;
+    return MMX_OK;
+  }
   const size_t old_cnt = vecN(w);
   const int old_nvec = w->nvec;
   float* oldY = w->Y[0] ? w->Y[w->sel_host] : nullptr;
@@ -204,6 +209,8 @@ int alloc_state(mmx_world* w) {
   }
   if (w->has_elastic && !w->strain)
     if (int rc = dev_alloc(w, &w->strain, 6 * w->N)) return rc;
+  if (w->has_elastic && w->el.rayleigh_beta != 0.0 && !w->strain_f)
+    if (int rc = dev_alloc(w, &w->strain_f, 6 * w->N)) return rc;
   w->sel_host = 0;
   w->k1_valid = false;
   w->cfg_epoch++;
@@ -264,6 +271,8 @@ void fill_elastic(const mmx_world* w, ElasticArgs& a) {
   a.face = w->el.traction_face;
   a.tamp = w->el.traction_amp; a.tfreq = w->el.traction_freq;
   a.strain = w->strain;
+  a.beta = (float)w->el.rayleigh_beta;
+  a.strain_f = w->el.rayleigh_beta != 0.0 ? w->strain_f : nullptr;
   a.vec_stride = 3 * w->N;
 }
 
@@ -569,7 +578,7 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
   memset(&w->dm, 0, sizeof(w->dm));
   w->Y[0] = w->Y[1] = w->YS[0] = w->YS[1] = nullptr;
   for (int i = 0; i <= MMX_MAX_STAGES; ++i) w->K[i] = nullptr;
-  w->bdemag = w->strain = w->scratch = nullptr;
+  w->bdemag = w->strain = w->strain_f = w->scratch = nullptr;
   w->d_ctrl = nullptr; w->d_acc = nullptr;
   w->sel_host = 0; w->k1_valid = false; w->k1_method = -1;
   w->dev_bytes = 0; w->launches = 0;
@@ -599,7 +608,7 @@ int mmx_world_destroy(mmx_world* w) {
   cudaFree(w->d_reg); cudaFree(w->d_mat); cudaFree(w->d_ctrl); cudaFree(w->d_acc);
   for (int i = 0; i < 2; ++i) { cudaFree(w->Y[i]); cudaFree(w->YS[i]); }
   for (int i = 0; i <= MMX_MAX_STAGES; ++i) cudaFree(w->K[i]);
-  cudaFree(w->bdemag); cudaFree(w->strain); cudaFree(w->scratch);
+  cudaFree(w->bdemag); cudaFree(w->strain); cudaFree(w->strain_f); cudaFree(w->scratch);
   for (int a = 0; a < 3; ++a) cudaFree(w->dm.tw[a]);
   cudaFree(w->dm.spec1); cudaFree(w->dm.spec2); cudaFree(w->dm.khat);
   if (w->step_graph) cudaGraphExecDestroy(w->step_graph);
@@ -680,6 +689,7 @@ int mmx_set_elastic(mmx_world* w, const mmx_elastic* e) {
   if (e) {
     if (!(e->rho > 0)) return mmx_fail(MMX_EINVAL, "rho must be > 0");
     if (e->traction_face < -1 || e->traction_face > 5) return mmx_fail(MMX_EINVAL, "traction_face out of range");
+    if (!(e->rayleigh_beta >= 0)) return mmx_fail(MMX_EINVAL, "rayleigh_beta must be >= 0");
     w->el = *e;
     w->has_elastic = true;
   } else {

@@ -74,6 +74,23 @@ __global__ void __launch_bounds__(256) k_strain(ElasticArgs a) {
   a.strain[3 * N + i] = 0.5f * (g[0][1] + g[1][0]);
   a.strain[4 * N + i] = 0.5f * (g[0][2] + g[2][0]);
   a.strain[5 * N + i] = 0.5f * (g[1][2] + g[2][1]);
+  if (a.strain_f) {
+    // viscous damping: "an extra term, proportional to the strain rate, is added to the total
+    // stress tensor"; stiffness-proportional Rayleigh form sigma = C : (eps(u) + beta eps(v)), so the
+    // force kernel takes its stress from the strain of u + beta v.  v follows u in the state vector.
+    const float* v = u + 3 * N;
+    float gv[3][3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) gv[ax][j] = grad1(v + (size_t)j * N + i, p[ax], n[ax], a.per[ax], st[ax], a.inv_h[ax]);
+    a.strain_f[i] = fmaf(a.beta, gv[0][0], g[0][0]);
+    a.strain_f[N + i] = fmaf(a.beta, gv[1][1], g[1][1]);
+    a.strain_f[2 * N + i] = fmaf(a.beta, gv[2][2], g[2][2]);
+    a.strain_f[3 * N + i] = 0.5f * (fmaf(a.beta, gv[0][1] + gv[1][0], g[0][1] + g[1][0]));
+    a.strain_f[4 * N + i] = 0.5f * (fmaf(a.beta, gv[0][2] + gv[2][0], g[0][2] + g[2][0]));
+    a.strain_f[5 * N + i] = 0.5f * (fmaf(a.beta, gv[1][2] + gv[2][1], g[1][2] + g[2][1]));
+  }
 }
 
 // sigma_ij at the cell whose strain components are e[6] = xx,yy,zz,xy,xz,yz
@@ -139,7 +156,7 @@ __global__ void __launch_bounds__(256) k_elastic(ElasticArgs a) {
     for (int ax = 0; ax < 3; ++ax) {
       const float flo = (a.face == 2 * ax) ? -tr[j] : 0.f;
       const float fhi = (a.face == 2 * ax + 1) ? tr[j] : 0.f;
-      f[j] += div1(a, a.strain, N, i, ax, j, p[ax], n[ax], a.per[ax], st[ax], a.inv_h[ax], flo, fhi);
+      f[j] += div1(a, a.strain_f ? a.strain_f : a.strain, N, i, ax, j, p[ax], n[ax], a.per[ax], st[ax], a.inv_h[ax], flo, fhi);
     }
   // f_mel (Eq.8), summed over sublattices
   const int rc = a.reg ? a.reg[i] : 0;

@@ -98,7 +98,9 @@ struct ElasticArgs {
   float tvec[3];
   double tamp, tfreq;
   const float* yin[2];
-  float* strain;   // [6][N]
+  float* strain;   // [6][N]  eps(u): magnetoelastic field, strain energy
+  float* strain_f; // [6][N]  eps(u) + beta eps(v): stress of the elastic force when beta != 0, else null
+  float beta;      // Rayleigh stiffness coefficient, s
   float* kout[2];
   float* accel_out;  // non-null: write the acceleration only
   int stage, n_prev;
@@ -159,6 +161,7 @@ struct mmx_world {
   float* K[MMX_MAX_STAGES + 1];
   float* bdemag;
   float* strain;
+  float* strain_f;     // [6][N], only with viscous elastic damping
   float* scratch;      // [3][N]
   MmxCtrl* d_ctrl;
   double* d_acc;       // fp64 accumulators for energies

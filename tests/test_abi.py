@@ -37,7 +37,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(binding.Material) == 20 * 8
     assert ctypes.sizeof(binding.Coupling) == 6 * 8
     assert ctypes.sizeof(binding.RkOpts) == 56 and ctypes.sizeof(binding.RkStats) == 56
-    assert ctypes.sizeof(binding.Elastic) == 80
+    assert ctypes.sizeof(binding.Elastic) == 88
 
 
 def test_no_cpu_fallback(lib):

@@ -269,3 +269,35 @@ def test_fast_path_bitwise_repeatable():
     assert np.array_equal(ma, mb)
     assert np.array_equal(a.get_err_history(10), b.get_err_history(10))
     a.destroy(); b.destroy()
+
+
+def test_viscous_elastic_damping_acceleration_and_trajectory():
+    """Rayleigh (stiffness-proportional) elastic damping, P:L177 / Table 1: sigma = C : (eps(u) +
+    beta eps(v)).  Acceleration parity on a random (u, v) with open and periodic axes, then a short
+    co-integrated DP45 trajectory of the c5 recipe with beta = 0.1 ps (the paper's NiO value)."""
+    for grid, pbc in [((40, 24, 1), (0, 0, 0)), ((32, 16, 1), (1, 0, 0)), ((12, 10, 6), (0, 0, 0))]:
+        spec = wl.make("c5", grid)
+        spec.pbc = pbc
+        spec.demag = False
+        spec.elastic["beta"] = 1e-13
+        rng = np.random.default_rng(17)
+        spec.u = (1e-12 * rng.standard_normal(spec.u.shape)).astype(np.float32)
+        spec.v = (1e1 * rng.standard_normal(spec.v.shape)).astype(np.float32)   # beta v ~ u
+        g, o = pair(spec)
+        ref = o.acceleration(o.m, o.u, 0.0, o.v)
+        undamped = o.acceleration(o.m, o.u, 0.0)
+        assert field_err(undamped, ref) > 1e-2          # the viscous term matters in this state
+        assert field_err(g.eval_accel(), ref) < FIELD_TOL, (grid, pbc)
+        g.destroy()
+    spec = wl.make("c5", (64, 32, 1))
+    spec.elastic["beta"] = 1e-13
+    dt = spec.integrator["dt"]
+    g, o = pair(spec)
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=100)
+    o.step_dp45_fixed(dt, 100)
+    for s_ in range(spec.S):
+        assert np.abs(g.get_state(mmx.F_M0 + s_).astype(np.float64) - o.m[s_]).max() <= 1e-4
+    u, v = g.get_state(mmx.F_U), g.get_state(mmx.F_V)
+    assert np.abs(u - o.u).max() <= 1e-4 * max(np.abs(o.u).max(), 1e-30)
+    assert np.abs(v - o.v).max() <= 1e-4 * max(np.abs(o.v).max(), 1e-30)
+    g.destroy()
