@@ -86,6 +86,16 @@ def homogeneous_exchange(m_other, Ms, A0, latcon):
 # ----------------------------------------------------------------------
 # Eq.4, interfacial subset (S7): D_xzx = D_yzy = +D, D_xxz = D_yyz = -D
 # ----------------------------------------------------------------------
+def dmi_homogeneous(m_other, Ms, d, s):
+    """Eq.6: energy density eps = d . (m^(s) x m^(s')) between the two sublattices of a
+    cell, d the DMI vector in J/m^3.  Reading S32: (s, s') = (first, second) sublattice.  Then
+    eps = m1 . (m2 x d) = m2 . (d x m1), so B^(1) = -(m2 x d)/Ms1 = (d x m2)/Ms1 and
+    B^(2) = -(d x m1)/Ms2 = (m1 x d)/Ms2.  `m_other` is the partner sublattice, `s` this one."""
+    dv = np.asarray(d, float).reshape(3, 1, 1, 1) * np.ones_like(m_other)
+    B = cross(dv, m_other) if s == 0 else cross(m_other, dv)
+    return B * _inv(Ms)[None]
+
+
 def dmi_interfacial(mq, Ms, D, cell, pbc):
     """B = sum_{n in +-x, +-y} D_cn / (Ms_c h_n) (z^ x e_cn) x mq_n ;
     continuum limit (2D/Ms)(dx m_z, dy m_z, -dx m_x - dy m_y)."""

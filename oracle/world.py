@@ -14,7 +14,7 @@ from . import elastic as el
 from . import fields as fl
 from . import newell as nw
 from . import rk
-from .constants import (T_A0, T_A12, T_ALL, T_ANIS_C, T_ANIS_U, T_DEMAG, T_DMI, T_DMI_INTER,
+from .constants import (T_A0, T_A12, T_ALL, T_ANIS_C, T_ANIS_U, T_DEMAG, T_DMI, T_DMI_HOMO, T_DMI_INTER,
                         T_EXCH, T_MEL, T_ZEEMAN)
 
 
@@ -105,6 +105,8 @@ class World:
             if terms & T_DMI_INTER:
                 Di = np.full_like(p["Ms"], self.cpl["D_inter"])
                 out[T_DMI_INTER] = fl.dmi_interfacial(m[o], p["Ms"], Di, self.cell, self.pbc)
+            if terms & T_DMI_HOMO:
+                out[T_DMI_HOMO] = fl.dmi_homogeneous(m[o], p["Ms"], self.cpl.get("d_homo", (0.0, 0.0, 0.0)), s)
         if (terms & T_MEL) and self.elastic is not None:
             u = self.u if u is None else u
             out[T_MEL] = fl.magnetoelastic_field(m[s], p["Ms"], p["B1"], p["B2"], self.strain(u))

@@ -154,6 +154,40 @@ def test_P12_antiferromagnetic_resonance():
     assert abs(f_got - f_want) < 2e-3 * f_want
 
 
+def test_P21_weak_ferromagnet_canting_angle():
+    """Two macrospins with antiferromagnetic homogeneous exchange eps = J m1.m2 (J = -4 A0/a^2 > 0) and
+    the homogeneous DMI of Eq.6 with d along z, eps_D = d z.(m1 x m2): for in-plane spins with
+    Delta = phi2 - phi1 the energy is J cos(Delta) + d sin(Delta), stationary where tan(Delta) = d/J
+    and minimal at Delta = pi + atan(d/J) (weak-ferromagnetic canting).  The oracle's torque must
+    vanish exactly there, its energy must be a minimum there, and the state canted the other way
+    must feel a torque.  (A relaxation run is not used: without anisotropy the out-of-plane mode of
+    this pair relaxes on a nanosecond scale.)"""
+    Ms, A0, a, dz = 4.0e5, -4.0e-13, 0.35e-9, 2.0e5
+    J = -4 * A0 / (a * a)
+    delta0 = np.arctan(dz / J)
+
+    def world(delta, phi1=0.3):
+        m1 = np.array([np.cos(phi1), np.sin(phi1), 0.0]).reshape(3, 1, 1, 1)
+        m2 = np.array([np.cos(phi1 + np.pi + delta), np.sin(phi1 + np.pi + delta), 0.0]).reshape(3, 1, 1, 1)
+        spec = wl.WorldSpec(name="wfm", grid=(1, 1, 1), cell=(2e-9,) * 3, S=2, demag=False,
+                            mat=wl.make_mat(2, Ms=Ms, alpha=0.5),
+                            coupling=wl.default_coupling(A0=A0, latcon=a, d_homo=(0.0, 0.0, dz)),
+                            m=[m1.astype(np.float32), m2.astype(np.float32)])
+        w = World(spec)
+        w.m = [m1, m2]
+        return w
+
+    scale = GAMMA * J / Ms                      # torque scale of the exchange field, 1/s
+    assert world(delta0).max_torque() < 1e-12 * scale
+    assert world(-delta0).max_torque() > 1e-3 * scale          # wrong chirality is not an equilibrium
+    assert world(0.0).max_torque() > 1e-3 * scale              # neither is the collinear state
+    e0 = world(delta0).energy()
+    for eps in (1e-3, -1e-3):
+        assert world(delta0 + eps).energy() > e0
+    V = (2e-9) ** 3
+    assert abs(e0 - V * (J * np.cos(np.pi + delta0) + dz * np.sin(np.pi + delta0))) < 1e-9 * abs(e0)
+
+
 def test_P13_zhang_li():
     """alpha = xi: the Zhang-Li torque reduces to the transverse part of (u.grad)m, with
     u = mu_B P j/(e Ms (1+xi^2)) (71.6 m/s for the c3 numbers); a wall translates rigidly at -u."""

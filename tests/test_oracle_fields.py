@@ -4,8 +4,8 @@ import pytest
 
 import workloads as wl
 from oracle import fields as fl
-from oracle.constants import (T_A0, T_A12, T_ANIS_C, T_ANIS_U, T_DEMAG, T_DMI, T_DMI_INTER, T_EXCH,
-                              T_MEL, T_ZEEMAN)
+from oracle.constants import (T_A0, T_A12, T_ANIS_C, T_ANIS_U, T_DEMAG, T_DMI, T_DMI_HOMO, T_DMI_INTER,
+                              T_EXCH, T_MEL, T_ZEEMAN)
 from oracle.world import World
 
 
@@ -74,7 +74,8 @@ def _toy_world(pbc, seed=3, elastic=False):
     spec = wl.WorldSpec(
         name="toy", grid=grid, cell=(2e-9, 2.5e-9, 1.5e-9), pbc=pbc, S=S,
         regions=rng.integers(0, R, (grid[2], grid[1], grid[0])).astype(np.uint16), mat=mat,
-        coupling=wl.default_coupling(A0=-4e-13, A12=-1e-12, D_inter=0.8e-3, scale_A11=0.25, scale_A12=0.5),
+        coupling=wl.default_coupling(A0=-4e-13, A12=-1e-12, D_inter=0.8e-3, scale_A11=0.25, scale_A12=0.5,
+                                     d_homo=(3e4, -2e4, 5e4)),
         bext=(0.05, -0.02, 0.1),
         elastic=dict(C11=2.5e11, C12=1.5e11, C44=1.0e11, rho=6800.0) if elastic else None,
         m=[wl.random_unit(rng, grid), wl.random_unit(rng, grid)],
@@ -85,7 +86,7 @@ def _toy_world(pbc, seed=3, elastic=False):
 
 @pytest.mark.parametrize("pbc", [(0, 0, 0), (1, 1, 0)])
 @pytest.mark.parametrize("term", [T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0,
-                                  T_DMI_INTER, T_MEL])
+                                  T_DMI_INTER, T_MEL, T_DMI_HOMO])
 def test_P10_field_is_energy_gradient(pbc, term):
     """B_term = -(1/(Ms V)) dE_term/dm (unconstrained derivative of the oracle's energy),
     including OPEN boundary pairs, region-pair scaling and two sublattices."""
@@ -136,3 +137,31 @@ def test_anisotropy_special_cases():
     # cubic: B_x = -(2Kc1/Ms) m_x (m_y^2 + m_z^2)
     Bc = fl.cubic(m, 8e5 * one, 1e4 * one, x, y)
     np.testing.assert_allclose(Bc.ravel(), [-(2e4 / 8e5) * 0.6 * 0.64, 0, -(2e4 / 8e5) * 0.8 * 0.36], atol=1e-18)
+
+
+def test_P21_homogeneous_dmi_is_the_gradient_of_eq6():
+    """Eq.6 defines the term by its energy density eps = d . (m1 x m2).  The oracle
+    implements the FIELD; here the paper's energy is written out and differentiated numerically:
+    B^(s) = -(1/(Ms V)) d/dm^(s) [ V sum_cells d . (m1 x m2) ].  Pins the form and both signs."""
+    w = _toy_world((0, 0, 0))
+    d = np.asarray(w.cpl["d_homo"], float)
+
+    def eq6_energy():
+        c = np.cross(np.moveaxis(w.m[0], 0, -1), np.moveaxis(w.m[1], 0, -1))
+        return w.V * float((c @ d).sum())
+
+    B = [w.field_terms(s, terms=T_DMI_HOMO)[T_DMI_HOMO] for s in range(2)]
+    scale = max(np.abs(B[0]).max(), np.abs(B[1]).max())
+    rng = np.random.default_rng(5)
+    for _ in range(12):
+        s, c = int(rng.integers(0, 2)), int(rng.integers(0, 3))
+        iz, iy, ix = (int(rng.integers(0, n)) for n in (3, 4, 5))
+        m0 = w.m[s][c, iz, iy, ix]
+        E = []
+        for sgn in (+1, -1):
+            w.m[s][c, iz, iy, ix] = m0 + sgn * 1e-4
+            E.append(eq6_energy())
+        w.m[s][c, iz, iy, ix] = m0
+        want = -(E[0] - E[1]) / 2e-4 / (w.p[s]["Ms"][iz, iy, ix] * w.V)
+        assert abs(B[s][c, iz, iy, ix] - want) < 1e-8 * scale, (s, c)
+    assert abs(w.energy(T_DMI_HOMO) - eq6_energy()) < 1e-10 * abs(eq6_energy())

@@ -78,7 +78,8 @@ def make_mat(S: int, R: int = 1, **kw) -> dict:
 
 
 def default_coupling(**kw) -> dict:
-    c = dict(A0=0.0, A12=0.0, latcon=0.35e-9, D_inter=0.0, scale_A11=1.0, scale_A12=1.0)
+    c = dict(A0=0.0, A12=0.0, latcon=0.35e-9, D_inter=0.0, scale_A11=1.0, scale_A12=1.0,
+             d_homo=(0.0, 0.0, 0.0))
     c.update(kw)
     return c
 
