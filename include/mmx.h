@@ -58,7 +58,8 @@ enum {
   MMX_T_A0 = 128,        /* Eq.3 third term: 4 A0/(a^2 Ms) m'                          */
   MMX_T_DMI_INTER = 256, /* Eq.4 with the inter-sublattice tensor                      */
   MMX_T_MEL = 512,       /* Eq.9 magnetoelastic field */
-  MMX_T_ALL = 1023
+  MMX_T_DMI_HOMO = 1024, /* Eq.6 homogeneous DMI between the sublattices */
+  MMX_T_ALL = 2047
 };
 
 /* state fields for mmx_set_state / mmx_get_state */
@@ -99,6 +100,8 @@ typedef struct mmx_coupling {
   double D_inter;   /* inter-sublattice interfacial DMI, J/m^2                         */
   double scale_A11; /* factor on A11 between cells of different regions (1 = none)     */
   double scale_A12; /* factor on A12 between cells of different regions                */
+  double d_homo[3]; /* DMI vector d of Eq.6, J/m^3: energy density d . (m1 x m2), m1 / m2 the  */
+                    /* first / second sublattice (the paper does not fix the order: a reading) */
 } mmx_coupling;
 
 /* Elastic medium (Eq.7) and one optional time-harmonic traction. */

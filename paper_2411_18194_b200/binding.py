@@ -15,9 +15,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmmx.so")
 
 HOST, DEVICE = 0, 1
-T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0, T_DMI_INTER, T_MEL = (
-    1, 2, 4, 8, 16, 32, 64, 128, 256, 512)
-T_ALL = 1023
+T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0, T_DMI_INTER, T_MEL, T_DMI_HOMO = (
+    1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1024)
+T_ALL = 2047
 F_M0, F_M1, F_U, F_V = 0, 1, 2, 3
 RK4, DP45, HEUN12, BS23, CK45, RKF45 = 0, 1, 2, 3, 4, 5
 FACES = {"x-": 0, "x+": 1, "y-": 2, "y+": 3, "z-": 4, "z+": 5}
@@ -40,7 +40,8 @@ class Material(C.Structure):
 
 
 class Coupling(C.Structure):
-    _fields_ = [(k, C.c_double) for k in ("A0", "A12", "latcon", "D_inter", "scale_A11", "scale_A12")]
+    _fields_ = [(k, C.c_double) for k in ("A0", "A12", "latcon", "D_inter", "scale_A11", "scale_A12")] + [
+        ("d_homo", C.c_double * 3)]
 
 
 class Elastic(C.Structure):
@@ -213,8 +214,10 @@ class World:
                 setattr(m, k, float(v))
         _check(self.lib.mmx_set_material(self.h, sublattice, region, C.byref(m)))
 
-    def set_coupling(self, A0=0.0, A12=0.0, latcon=0.35e-9, D_inter=0.0, scale_A11=1.0, scale_A12=1.0):
+    def set_coupling(self, A0=0.0, A12=0.0, latcon=0.35e-9, D_inter=0.0, scale_A11=1.0, scale_A12=1.0,
+                     d_homo=(0.0, 0.0, 0.0)):
         c = Coupling(A0, A12, latcon, D_inter, scale_A11, scale_A12)
+        c.d_homo[:] = [float(x) for x in d_homo]
         _check(self.lib.mmx_set_coupling(self.h, C.byref(c)))
 
     def set_bext(self, B):

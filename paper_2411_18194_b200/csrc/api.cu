@@ -225,7 +225,7 @@ unsigned active_terms(const mmx_world* w) {
   unsigned t = MMX_T_ALL;
   if (!(w->use_demag && w->dm.ready)) t &= ~MMX_T_DEMAG;
   if (!w->has_elastic) t &= ~MMX_T_MEL;
-  if (w->S != 2) t &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER);
+  if (w->S != 2) t &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER | MMX_T_DMI_HOMO);
   return t;
 }
 
@@ -247,6 +247,7 @@ void fill_local(const mmx_world* w, LocalArgs& a, unsigned terms) {
   a.A12 = (float)w->cpl.A12;
   a.a0pref = (float)(w->cpl.latcon > 0 ? 4.0 * w->cpl.A0 / (w->cpl.latcon * w->cpl.latcon) : 0.0);
   a.Dinter = (float)w->cpl.D_inter;
+  for (int k = 0; k < 3; ++k) a.dhomo[k] = (float)w->cpl.d_homo[k];
   a.terms = terms;
   a.has_J = (w->J[0] != 0.0 || w->J[1] != 0.0 || w->J[2] != 0.0) ? 1 : 0;
   a.bdemag = (terms & MMX_T_DEMAG) ? w->bdemag : nullptr;
@@ -832,7 +833,7 @@ int mmx_eval_heff(mmx_world* w, int sublattice, unsigned term_mask, float* out, 
   if (int rc = prepare(w)) return rc;
   unsigned terms = term_mask;
   if (!w->has_elastic) terms &= ~MMX_T_MEL;
-  if (w->S != 2) terms &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER);
+  if (w->S != 2) terms &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER | MMX_T_DMI_HOMO);
   if (int rc = eval_prereq(w, terms)) return rc;
   LocalArgs la;
   fill_local(w, la, terms);
@@ -889,7 +890,7 @@ int mmx_energy(mmx_world* w, unsigned term_mask, double* joule_out) {
   int slot = 0;
   double coef[64];
   for (int s = 0; s < w->S; ++s)
-    for (int b = 0; b < 10; ++b) {
+    for (int b = 0; b < 11; ++b) {  // one pass per term bit of MMX_T_ALL
       const unsigned bit = 1u << b;
       if (!(terms & bit)) continue;
       LocalArgs la;

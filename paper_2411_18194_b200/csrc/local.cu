@@ -5,6 +5,7 @@
 //   B_exch  = sum_n 2 A_cn /(Ms_c h_n^2) (m_n - m_c)                  Eq.3 term 1
 //   B_A12   = sum_n A12_cn /(Ms_c h_n^2) (m'_n - m'_c)                Eq.3 term 2
 //   B_A0    = 4 A0 /(a^2 Ms_c) m'_c                                    Eq.3 term 3
+//   B_Dhom  = (d x m2)/Ms1 on sublattice 1, (m1 x d)/Ms2 on sublattice 2      Eq.6
 //   B_DMI   = sum_{n in +-x,+-y} D_cn /(Ms_c h_n) (z x e_cn) x m_n     Eq.4, interfacial subset
 //   B_anis  = 2Ku1/Ms (u.m) u  - 2Kc1/Ms sum_i (c_i.m)[(c_j.m)^2+(c_k.m)^2] c_i
 //   B_mel   = -2/Ms [B1 eps_ii m_i + B2 (eps_ij m_j + eps_ik m_k)]     Eq.9
@@ -163,6 +164,11 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
           }
         }
         if (S == 2 && (a.terms & MMX_T_A0)) B = fma3(a.a0pref * iMs, mc[o], B);
+        if (S == 2 && (a.terms & MMX_T_DMI_HOMO)) {
+          // Eq.6: eps = d . (m1 x m2)  =>  B1 = (d x m2)/Ms1,  B2 = (m1 x d)/Ms2
+          const V3 dv = v3(a.dhomo[0], a.dhomo[1], a.dhomo[2]);
+          B = fma3(iMs, s == 0 ? cross(dv, mc[o]) : cross(mc[o], dv), B);
+        }
         if (a.terms & MMX_T_ANIS_U) {
           const V3 u = v3(P[MP_UX], P[MP_UY], P[MP_UZ]);
           B = fma3(P[MP_KU2] * dot(u, mc[s]), u, B);
@@ -460,6 +466,10 @@ __global__ void __launch_bounds__(MMX_L4_BLOCK, MMX_L4_MINB) k_local4(LocalArgs 
         const V3 m = mc[s].c[e];
         V3 Bc = B.c[e];
         if (S == 2 && (a.terms & MMX_T_A0)) Bc = fma3(a.a0pref * iMs, mc[o].c[e], Bc);
+        if (S == 2 && (a.terms & MMX_T_DMI_HOMO)) {
+          const V3 dv = v3(a.dhomo[0], a.dhomo[1], a.dhomo[2]);
+          Bc = fma3(iMs, s == 0 ? cross(dv, mc[o].c[e]) : cross(mc[o].c[e], dv), Bc);
+        }
         if (a.terms & MMX_T_ANIS_U) {
           const V3 u = v3(P[MP_UX], P[MP_UY], P[MP_UZ]);
           Bc = fma3(P[MP_KU2] * dot(u, m), u, Bc);

@@ -62,6 +62,7 @@ struct LocalArgs {
   const uint16_t* reg;   // null when nreg == 1
   const float* mat;      // [S][nreg][MMX_MATW]
   float scaleA11, scaleA12, A12, a0pref, Dinter;
+  float dhomo[3];        // DMI vector of Eq.6, J/m^3
   float bext[3], J[3];
   unsigned terms;
   int has_J;

@@ -164,3 +164,34 @@ def test_graph_replay_equals_plain_launches_and_follows_parameter_changes():
     assert a.graph_info() > 0
     assert np.array_equal(a.get_state(mmx.F_M0), b.get_state(mmx.F_M0))
     a.destroy(); b.destroy()
+
+
+def test_weak_ferromagnet_canting_is_an_equilibrium_of_the_cuda_path():
+    """Eq.6 closed form, end to end on the GPU: with antiferromagnetic homogeneous exchange
+    J = -4 A0/a^2 and d along z the state canted by atan(d/J) has no torque; the state canted the
+    other way has (reading S32 fixes which one is which)."""
+    Ms, A0, a, dz = 4.0e5, -4.0e-13, 0.35e-9, 2.0e5
+    J = -4 * A0 / (a * a)
+    delta0 = np.arctan(dz / J)
+    scale = 1.7595e11 * J / Ms
+    tq = {}
+    for name, delta in (("right", delta0), ("wrong", -delta0)):
+        spec = wl.make("c3", (8, 4, 1))
+        spec.regions = None
+        for k, v in spec.mat.items():
+            spec.mat[k] = v[:, :1].copy()
+        spec.mat["Ms"][:] = Ms
+        spec.mat["Ku1"][:] = 0.0
+        spec.mat["D"][:] = 0.0
+        spec.J = (0.0, 0.0, 0.0)
+        spec.demag = False
+        spec.coupling.update(A0=A0, A12=0.0, D_inter=0.0, latcon=a, d_homo=(0.0, 0.0, dz))
+        phi1 = 0.3
+        for s, phi in ((0, phi1), (1, phi1 + np.pi + delta)):
+            spec.m[s][:] = 0
+            spec.m[s][0], spec.m[s][1] = np.cos(phi), np.sin(phi)
+        g = mmx.World.from_spec(spec)
+        tq[name] = g.max_torque()
+        g.destroy()
+    assert tq["right"] < 1e-5 * scale, tq      # fp32: cancellation of two ~33 T fields
+    assert tq["wrong"] > 1e-3 * scale, tq

@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 
 TERMS = {"exch": mmx.T_EXCH, "dmi": mmx.T_DMI, "anis_u": mmx.T_ANIS_U, "anis_c": mmx.T_ANIS_C,
          "zeeman": mmx.T_ZEEMAN, "demag": mmx.T_DEMAG, "a12": mmx.T_A12, "a0": mmx.T_A0,
-         "dmi_inter": mmx.T_DMI_INTER, "mel": mmx.T_MEL}
+         "dmi_inter": mmx.T_DMI_INTER, "mel": mmx.T_MEL, "dmi_homo": mmx.T_DMI_HOMO}
 
 
 def _rich_spec(name, grid, seed=7):
@@ -31,7 +31,8 @@ def _rich_spec(name, grid, seed=7):
         spec.mat["A"][s] = 1e-11 * (1 + 0.3 * rng.random(R))
     spec.bext = (0.01, -0.02, 0.1)
     if spec.S == 2:
-        spec.coupling.update(A0=-4e-13, A12=-1e-12, D_inter=0.5e-3, scale_A11=0.25, scale_A12=0.5)
+        spec.coupling.update(A0=-4e-13, A12=-1e-12, D_inter=0.5e-3, scale_A11=0.25, scale_A12=0.5,
+                             d_homo=(3e4, -2e4, 5e4))
     return spec
 
 
