@@ -129,12 +129,18 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_q(InnerColArgs a) {
       const int kom = (a.p_outer > 1 && 2 * ko > a.p_outer) ? a.p_outer - ko : ko;
       const int kx0 = (tile - (tile / a.ntile_main) * a.ntile_main) * TL;
       const unsigned kb = (unsigned)kom * (unsigned)a.k_outer_stride + (unsigned)kx0;
-      for (int q = threadIdx.x; q < 6 * (H + 1) * (TL / 4); q += NT) {
-        const int row = q / (TL / 4), ch = q % (TL / 4);
-        const int c = row / (H + 1), pm = row - c * (H + 1);
-        const unsigned sa = (unsigned)__cvta_generic_to_shared(kst + row * TL + 4 * ch);
-        const float* g = a.khat + (kb + (unsigned)c * (unsigned)a.k_comp_stride + (unsigned)pm * (unsigned)a.k_inner_stride + 4 * ch);
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(g) : "memory");
+      // rows (c, pm) are equidistant in the octant when k_comp_stride = (H + 1) k_inner_stride (the
+      // launcher checks it): row r = c (H + 1) + pm sits at r * k_inner_stride, no division by H + 1
+      const unsigned kis = (unsigned)a.k_inner_stride;
+#pragma unroll
+      for (int q0 = 0; q0 < 6 * (H + 1) * (TL / 4); q0 += NT) {
+        const int q = q0 + threadIdx.x;
+        if (q < 6 * (H + 1) * (TL / 4)) {
+          const unsigned row = q / (TL / 4), ch = q % (TL / 4);
+          const unsigned sa = (unsigned)__cvta_generic_to_shared(kst + row * TL + 4 * ch);
+          const float* g = a.khat + (kb + row * kis + 4 * ch);
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(g) : "memory");
+        }
       }
     } else {
       const int ko0 = (tile - ntm) * TL;
@@ -524,6 +530,8 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
   a.k_inner_stride = L.k_inner_stride; a.k_outer_stride = L.k_outer_stride; a.k_comp_stride = L.k_comp_stride;
   a.odd_inner = L.odd_inner; a.odd_outer = L.odd_outer;
   if (L.p_outer != L.n_outer) return mmx_fail(MMX_EINVAL, "inner column pass: outer extent mismatch");
+  if (L.k_comp_stride != (size_t)65 * L.k_inner_stride)
+    return mmx_fail(MMX_EINVAL, "inner column pass: kernel octant rows are not equidistant");
   if (3 * L.comp_stride >= (1ull << 31) || 6 * L.k_comp_stride >= (1ull << 31))
     return mmx_fail(MMX_EINVAL, "inner column pass: spectra exceed the 32-bit element offsets of this kernel");
   ProfScope ps(w, PK_INNER);
