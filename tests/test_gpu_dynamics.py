@@ -195,3 +195,36 @@ def test_weak_ferromagnet_canting_is_an_equilibrium_of_the_cuda_path():
         g.destroy()
     assert tq["right"] < 1e-5 * scale, tq      # fp32: cancellation of two ~33 T fields
     assert tq["wrong"] > 1e-3 * scale, tq
+
+
+def test_c4_full_size_invariants_of_the_trajectory():
+    """BASELINE config 4 at full size (256x256x64, the launch configuration bench.py times).  The
+    oracle cannot follow a trajectory at this size, so properties that hold at any size are checked
+    (P8, P9): |m| = 1 after every call, the total energy falls monotonically (alpha = 0.1 > 0), and the
+    energy lost equals the dissipated power  P = (alpha Ms V / gamma) sum_c |tau_c|^2  integrated by
+    the trapezoid rule over short stretches (dE/dt = -alpha gamma/(1+alpha^2) sum Ms V |m x B|^2)."""
+    spec = wl.make("c4")
+    assert tuple(spec.grid) == (256, 256, 64)
+    g = mmx.World.from_spec(spec)
+    Ms, alpha, gamma = float(spec.mat["Ms"][0, 0]), float(spec.mat["alpha"][0, 0]), 1.7595e11
+    V = float(np.prod(spec.cell))
+
+    def power():
+        tau = g.eval_torque(0).astype(np.float64)
+        return alpha * Ms * V / gamma * float((tau ** 2).sum())
+
+    dt, n = 2e-14, 4
+    E = [g.energy()]
+    P = [power()]
+    for _ in range(3):
+        st = g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=n)
+        assert st["accepted"] == n
+        m = g.get_state(mmx.F_M0).astype(np.float64)
+        np.testing.assert_allclose((m ** 2).sum(axis=0), 1.0, atol=2e-6)
+        E.append(g.energy())
+        P.append(power())
+        assert E[-1] < E[-2]
+        lost = E[-2] - E[-1]
+        trapezoid = 0.5 * (P[-2] + P[-1]) * n * dt
+        assert abs(lost - trapezoid) < 0.02 * lost, (lost, trapezoid)
+    g.destroy()
