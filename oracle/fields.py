@@ -96,6 +96,33 @@ def dmi_homogeneous(m_other, Ms, d, s):
     return B * _inv(Ms)[None]
 
 
+def dmi_tensor(mq, Ms, q, cell, pbc):
+    """General DMI of Eq.4 for s = s': eps = sum_ijk D_ijk m_j d_i m_k with
+    D_ijk = -D_ikj, "9 independent components".  For each axis i the antisymmetric 3x3 block is a
+    vector q_i, D_ijk = sum_l eps_jkl q_il, so eps = sum_i q_i . (m x d_i m) and
+    B = -(1/Ms) delta E/delta m = (2/Ms) sum_i q_i x d_i m.  Discretised pair by pair like the
+    interfacial term (central difference; a pair whose partner is absent or has Ms = 0 adds
+    nothing, reading S9):  B_c = sum_i sum_{d=+-1} d / (Ms_c h_i) q_i x m_(c + d e_i).
+    q: [3 axes][3] in J/m^2, uniform (reading S33).  Interfacial D is q_x = D y^, q_y = -D x^;
+    bulk (Bloch) DMI eps = D m.(curl m) is q_i = -D e_i
+    (m.(curl m) = -sum_i e_i.(m x d_i m))."""
+    B = np.zeros_like(mq)
+    iMs = _inv(Ms)
+    q = np.asarray(q, float)
+    for axis in range(3):
+        if not np.any(q[axis]):
+            continue
+        h = cell[axis]
+        qv = q[axis].reshape(3, 1, 1, 1) * np.ones_like(mq)
+        for d in (+1, -1):
+            mn, ex = neighbour(mq, axis, d, pbc[axis] > 0)
+            Msn, _ = neighbour(Ms, axis, d, pbc[axis] > 0)
+            ok = ex & (Msn > 0) & (Ms > 0)
+            w = np.where(ok, iMs / h, 0.0) * d
+            B += w[None] * cross(qv, mn)
+    return B
+
+
 def dmi_interfacial(mq, Ms, D, cell, pbc):
     """B = sum_{n in +-x, +-y} D_cn / (Ms_c h_n) (z^ x e_cn) x mq_n ;
     continuum limit (2D/Ms)(dx m_z, dy m_z, -dx m_x - dy m_y)."""

@@ -87,6 +87,9 @@ class World:
                                             self.cell, self.pbc, 2.0)
         if terms & T_DMI:
             out[T_DMI] = fl.dmi_interfacial(m[s], p["Ms"], p["D"], self.cell, self.pbc)
+            q = self.cpl.get("dmi_q")
+            if q is not None and np.any(np.asarray(q)[s]):   # general tensor of Eq.4, same term bit
+                out[T_DMI] = out[T_DMI] + fl.dmi_tensor(m[s], p["Ms"], np.asarray(q)[s], self.cell, self.pbc)
         if terms & T_ANIS_U:
             out[T_ANIS_U] = fl.uniaxial(m[s], p["Ms"], p["Ku1"], p["u"])
         if terms & T_ANIS_C:

@@ -165,3 +165,74 @@ def test_P21_homogeneous_dmi_is_the_gradient_of_eq6():
         want = -(E[0] - E[1]) / 2e-4 / (w.p[s]["Ms"][iz, iy, ix] * w.V)
         assert abs(B[s][c, iz, iy, ix] - want) < 1e-8 * scale, (s, c)
     assert abs(w.energy(T_DMI_HOMO) - eq6_energy()) < 1e-10 * abs(eq6_energy())
+
+
+def _dijk_from_q(q):
+    """D_ijk = sum_l eps_jkl q_il (antisymmetric in j, k): the paper's rank-3 tensor from the three
+    per-axis vectors."""
+    eps = np.zeros((3, 3, 3))
+    eps[0, 1, 2] = eps[1, 2, 0] = eps[2, 0, 1] = 1.0
+    eps[0, 2, 1] = eps[2, 1, 0] = eps[1, 0, 2] = -1.0
+    return np.einsum("jkl,il->ijk", eps, np.asarray(q, float))
+
+
+def test_P22_general_dmi_tensor_is_the_gradient_of_eq4():
+    """Eq.4 for s = s': eps = sum_ijk D_ijk m_j d_i m_k, D_ijk = -D_ikj, 9 independent
+    components.  The paper's energy is written out on a periodic grid with central differences and
+    differentiated numerically; the oracle's field must be its gradient.  Pins form, signs, the
+    factor 2 and the mapping D_ijk <-> q_i (reading S33)."""
+    rng = np.random.default_rng(21)
+    n = (6, 5, 4)                                   # (nx, ny, nz)
+    cell = (2e-9, 2.5e-9, 1.5e-9)
+    q = 1e-3 * rng.standard_normal((3, 3))
+    D = _dijk_from_q(q)
+    assert np.allclose(D, -np.swapaxes(D, 1, 2))
+    m = rng.standard_normal((3, n[2], n[1], n[0]))
+    Ms = 5e5 * np.ones(m.shape[1:])
+    V = float(np.prod(cell))
+
+    def eq4_energy(mm):
+        E = 0.0
+        for i in range(3):
+            ax = 3 - i                               # array axis of spatial axis i in [3, z, y, x]
+            dm = (np.roll(mm, -1, axis=ax) - np.roll(mm, 1, axis=ax)) / (2 * cell[i])
+            E += np.einsum("jk,jzyx,kzyx->", D[i], mm, dm)
+        return V * E
+
+    B = fl.dmi_tensor(m, Ms, q, cell, (1, 1, 1))
+    scale = np.abs(B).max()
+    for _ in range(15):
+        c = int(rng.integers(0, 3))
+        iz, iy, ix = (int(rng.integers(0, k)) for k in (n[2], n[1], n[0]))
+        m0 = m[c, iz, iy, ix]
+        E = []
+        for sgn in (+1, -1):
+            m[c, iz, iy, ix] = m0 + sgn * 1e-4
+            E.append(eq4_energy(m))
+        m[c, iz, iy, ix] = m0
+        want = -(E[0] - E[1]) / 2e-4 / (Ms[iz, iy, ix] * V)
+        assert abs(B[c, iz, iy, ix] - want) < 1e-7 * scale, c
+
+
+def test_P22_bulk_dmi_helix_closed_form_and_interfacial_special_case():
+    """Bulk (Bloch) DMI eps = D m.(curl m): since m.(curl m) = -sum_i e_i.(m x d_i m) this is
+    q_i = -D e_i.  For the helix m = (0, cos kx, sin kx), curl m = -k m, so
+    B = -(2D/Ms) curl m -> (2D/Ms)(sin kh / h) m on the grid.  And with q_x = D y^,
+    q_y = -D x^ the general term must reproduce the interfacial one cell by cell (open edges too)."""
+    nx, h, D, Ms = 32, 2e-9, 1.2e-3, 6e5
+    k = 2 * np.pi * 3 / (nx * h)
+    x = (np.arange(nx) + 0.5) * h
+    m = np.zeros((3, 1, 1, nx))
+    m[1, 0, 0], m[2, 0, 0] = np.cos(k * x), np.sin(k * x)
+    one = Ms * np.ones((1, 1, nx))
+    B = fl.dmi_tensor(m, one, -D * np.eye(3), (h, h, h), (1, 0, 0))
+    np.testing.assert_allclose(B, (2 * D / Ms) * np.sin(k * h) / h * m, atol=1e-12 * np.abs(B).max())
+    rng = np.random.default_rng(4)
+    mm = rng.standard_normal((3, 3, 5, 6))
+    Msr = 5e5 * np.ones(mm.shape[1:])
+    Msr[1, 2, 3] = 0.0                              # a hole: its pairs drop out in both forms
+    qi = np.array([[0, D, 0], [-D, 0, 0], [0, 0, 0]], float)
+    for pbc in [(0, 0, 0), (1, 1, 0)]:
+        a = fl.dmi_tensor(mm, Msr, qi, (2e-9, 3e-9, 1e-9), pbc)
+        b = fl.dmi_interfacial(mm, Msr, D * np.ones_like(Msr), (2e-9, 3e-9, 1e-9), pbc)
+        np.testing.assert_allclose(a, b, atol=1e-12 * np.abs(b).max())

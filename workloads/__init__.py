@@ -79,7 +79,7 @@ def make_mat(S: int, R: int = 1, **kw) -> dict:
 
 def default_coupling(**kw) -> dict:
     c = dict(A0=0.0, A12=0.0, latcon=0.35e-9, D_inter=0.0, scale_A11=1.0, scale_A12=1.0,
-             d_homo=(0.0, 0.0, 0.0))
+             d_homo=(0.0, 0.0, 0.0), dmi_q=None)   # dmi_q: [S][3][3] per-axis DMI vectors of Eq.4, J/m^2
     c.update(kw)
     return c
 
