@@ -170,6 +170,12 @@ int mmx_set_material(mmx_world* w, int sublattice, int region, const mmx_materia
 int mmx_set_coupling(mmx_world* w, const mmx_coupling* c);
 int mmx_set_bext(mmx_world* w, const double B[3]);     /* uniform external field, T */
 int mmx_set_current(mmx_world* w, const double J[3]);  /* Zhang-Li current density, A/m^2 */
+/* General intra-sublattice DMI of Eq.4: eps = sum_ijk D_ijk m_j d_i m_k, D_ijk = -D_ikj
+ * (9 independent components).  q[3*i + l] is component l of the vector q_i of axis i, J/m^2, with
+ * D_ijk = sum_l eps_jkl q_il, i.e. eps = sum_i q_i . (m x d_i m).  Uniform over the magnet; added to
+ * the interfacial term of mmx_material.D under the same term bit MMX_T_DMI.  Interfacial D equals
+ * q_x = D y^, q_y = -D x^; bulk DMI eps = D m.(curl m) equals q_i = -D e_i.  q = NULL clears it. */
+int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]);
 /* Enable elastodynamics (adds the fields U, V to the integrated state); NULL disables. */
 int mmx_set_elastic(mmx_world* w, const mmx_elastic* e);
 /* Switch the magnetostatic term on/off for stepping (default on once the kernel exists). */

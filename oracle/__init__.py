@@ -13,7 +13,7 @@ Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline /
 
 Pin status (see tests/test_oracle_*.py and DESIGN.md section "Oracle pins"):
   newell / demag .......... pinned (P1-P5, P19, mpmath spot values, dipole limit)
-  exchange, DMI, anisotropy pinned (P6, P10, P11)
+  exchange, DMI, anisotropy pinned (P6, P10, P11; general DMI tensor of Eq.4: P22)
   sublattice exchange ..... pinned (P10, P12); homogeneous DMI Eq.6 pinned (P21)
   LLG torque, integrators . pinned (P7, P8, P9, P14)
   Zhang-Li torque ......... pinned (P13: Gilbert-form identity, rigid translation at -u)

@@ -76,6 +76,7 @@ PROTOTYPES = {
     "mmx_set_coupling": (C.c_int, [_W, C.POINTER(Coupling)]),
     "mmx_set_bext": (C.c_int, [_W, _D3]),
     "mmx_set_current": (C.c_int, [_W, _D3]),
+    "mmx_set_dmi_tensor": (C.c_int, [_W, C.c_int, C.POINTER(C.c_double)]),
     "mmx_set_elastic": (C.c_int, [_W, C.POINTER(Elastic)]),
     "mmx_enable_demag": (C.c_int, [_W, C.c_int]),
     "mmx_set_state": (C.c_int, [_W, C.c_int, C.c_void_p, C.c_int]),
@@ -223,6 +224,14 @@ class World:
     def set_bext(self, B):
         _check(self.lib.mmx_set_bext(self.h, _arr(C.c_double, [float(x) for x in B])))
 
+    def set_dmi_tensor(self, sublattice, q):
+        """q: [3][3] per-axis DMI vectors of Eq.4 (J/m^2) or None to clear."""
+        if q is None:
+            _check(self.lib.mmx_set_dmi_tensor(self.h, int(sublattice), None))
+            return
+        flat = [float(x) for x in np.asarray(q, dtype=np.float64).reshape(9)]
+        _check(self.lib.mmx_set_dmi_tensor(self.h, int(sublattice), _arr(C.c_double, flat)))
+
     def set_current(self, J):
         _check(self.lib.mmx_set_current(self.h, _arr(C.c_double, [float(x) for x in J])))
 
@@ -360,7 +369,12 @@ class World:
                 kw = {k: spec.mat[k][s, r] for k in scal}
                 kw.update({k: spec.mat[k][s, r] for k in vecs})
                 w.set_material(s, r, **kw)
-        w.set_coupling(**spec.coupling)
+        cpl = dict(spec.coupling)
+        dmi_q = cpl.pop("dmi_q", None)
+        w.set_coupling(**cpl)
+        if dmi_q is not None:
+            for s in range(spec.S):
+                w.set_dmi_tensor(s, np.asarray(dmi_q)[s])
         w.set_bext(spec.bext)
         w.set_current(spec.J)
         if spec.elastic is not None:

@@ -248,6 +248,9 @@ void fill_local(const mmx_world* w, LocalArgs& a, unsigned terms) {
   a.a0pref = (float)(w->cpl.latcon > 0 ? 4.0 * w->cpl.A0 / (w->cpl.latcon * w->cpl.latcon) : 0.0);
   a.Dinter = (float)w->cpl.D_inter;
   for (int k = 0; k < 3; ++k) a.dhomo[k] = (float)w->cpl.d_homo[k];
+  a.has_dmiq = w->has_dmiq ? 1 : 0;
+  for (int s = 0; s < 2; ++s)
+    for (int k = 0; k < 9; ++k) a.dmiq[s][k / 3][k % 3] = (float)w->dmiq[s][k];
   a.terms = terms;
   a.has_J = (w->J[0] != 0.0 || w->J[1] != 0.0 || w->J[2] != 0.0) ? 1 : 0;
   a.bdemag = (terms & MMX_T_DEMAG) ? w->bdemag : nullptr;
@@ -553,6 +556,9 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
     if (cudaStreamCreate(&w->stream) == cudaSuccess) w->own_stream = true;
     else { cudaGetLastError(); w->stream = nullptr; }
   }
+  w->has_dmiq = false;
+  for (int s = 0; s < 2; ++s)
+    for (int k = 0; k < 9; ++k) w->dmiq[s][k] = 0.0;
   w->step_graph = nullptr; w->graph_method = -1; w->graph_epoch = -1; w->cfg_epoch = 0; w->graph_launches = 0;
   w->use_graphs = getenv("MMX_NO_GRAPH") == nullptr;
   {
@@ -680,6 +686,18 @@ int mmx_set_bext(mmx_world* w, const double B[3]) {
 int mmx_set_current(mmx_world* w, const double J[3]) {
   if (!w || !J) return mmx_fail(MMX_EINVAL, "NULL argument");
   for (int a = 0; a < 3; ++a) w->J[a] = J[a];
+  w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
+  return MMX_OK;
+}
+
+int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]) {
+  if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
+  if (sublattice < 0 || sublattice >= w->S) return mmx_fail(MMX_EINVAL, "sublattice %d out of range", sublattice);
+  for (int k = 0; k < 9; ++k) w->dmiq[sublattice][k] = q ? q[k] : 0.0;
+  w->has_dmiq = false;
+  for (int s = 0; s < 2; ++s)
+    for (int k = 0; k < 9; ++k) w->has_dmiq = w->has_dmiq || w->dmiq[s][k] != 0.0;
   w->k1_valid = false;
   w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;

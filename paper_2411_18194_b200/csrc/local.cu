@@ -7,6 +7,7 @@
 //   B_A0    = 4 A0 /(a^2 Ms_c) m'_c                                    Eq.3 term 3
 //   B_Dhom  = (d x m2)/Ms1 on sublattice 1, (m1 x d)/Ms2 on sublattice 2      Eq.6
 //   B_DMI   = sum_{n in +-x,+-y} D_cn /(Ms_c h_n) (z x e_cn) x m_n     Eq.4, interfacial subset
+//           + sum_i sum_{+-} +-1/(Ms_c h_i) q_i x m_n                   Eq.4, general tensor (k_local only)
 //   B_anis  = 2Ku1/Ms (u.m) u  - 2Kc1/Ms sum_i (c_i.m)[(c_j.m)^2+(c_k.m)^2] c_i
 //   B_mel   = -2/Ms [B1 eps_ii m_i + B2 (eps_ij m_j + eps_ik m_k)]     Eq.9
 //   B_eff   = sum of the above + B_ext + B_demag
@@ -140,6 +141,11 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
                 // (z x (d e_axis)) x m_n = d (m_z e_axis - m_axis z)
                 if (axis == 0) { B.x = fmaf(wd, mn.z, B.x); B.z = fmaf(-wd, mn.x, B.z); }
                 else { B.y = fmaf(wd, mn.z, B.y); B.z = fmaf(-wd, mn.y, B.z); }
+              }
+              if (a.has_dmiq && (a.terms & MMX_T_DMI)) {
+                // general tensor of Eq.4: B_c += d /(Ms_c h_i) q_i x m_n
+                const V3 qv = v3(a.dmiq[s][axis][0], a.dmiq[s][axis][1], a.dmiq[s][axis][2]);
+                B = fma3(iMs * a.inv_h[axis] * d, cross(qv, mn), B);
               }
               if (S == 2) {
                 if (a.terms & (MMX_T_A12 | MMX_T_DMI_INTER)) {
@@ -682,7 +688,7 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   const unsigned blocks = (unsigned)((N + 255) / 256);
   const bool reg = w->nreg > 1;
   ProfScope ps(w, PK_LOCAL);
-  bool uniform = !reg && (w->grid[0] % 4) == 0;
+  bool uniform = !reg && (w->grid[0] % 4) == 0 && !a.has_dmiq;  // (the general DMI tensor lives in k_local only)
   for (int s = 0; s < w->S && uniform; ++s) uniform = w->mats[(size_t)s * w->nreg].Ms > 0;
   if (uniform) {
     const unsigned b4 = (unsigned)((N / 4 + MMX_L4_BLOCK - 1) / MMX_L4_BLOCK);

@@ -63,6 +63,8 @@ struct LocalArgs {
   const float* mat;      // [S][nreg][MMX_MATW]
   float scaleA11, scaleA12, A12, a0pref, Dinter;
   float dhomo[3];        // DMI vector of Eq.6, J/m^3
+  float dmiq[2][3][3];   // general DMI tensor of Eq.4 as per-axis vectors q_i per sublattice, J/m^2
+  int has_dmiq;
   float bext[3], J[3];
   unsigned terms;
   int has_J;
@@ -152,6 +154,8 @@ struct mmx_world {
   bool mat_dirty;
   mmx_coupling cpl;
   double bext[3], J[3];
+  double dmiq[2][9];   // general DMI tensor (mmx_set_dmi_tensor), zero = none
+  bool has_dmiq;
   bool has_elastic;
   mmx_elastic el;
   bool use_demag;

@@ -302,3 +302,36 @@ def test_viscous_elastic_damping_acceleration_and_trajectory():
     assert np.abs(u - o.u).max() <= 1e-4 * max(np.abs(o.u).max(), 1e-30)
     assert np.abs(v - o.v).max() <= 1e-4 * max(np.abs(o.v).max(), 1e-30)
     g.destroy()
+
+
+@pytest.mark.parametrize("name,grid,pbc", [("c2", (32, 32, 1), (2, 2, 0)), ("c3", (48, 24, 1), (0, 0, 0)),
+                                           ("c4", (20, 12, 6), (0, 0, 0))])
+def test_general_dmi_tensor(name, grid, pbc):
+    """Eq.4, general antisymmetric tensor as per-axis vectors q_i (reading S33), added to
+    the interfacial term under the same term bit: field parity per sublattice (regions, holes,
+    open / periodic, 3-D), the total field, the torque, the energy, and a short trajectory."""
+    spec = _rich_spec(name, grid, seed=23)
+    spec.pbc = pbc
+    rng = np.random.default_rng(31)
+    spec.coupling["dmi_q"] = 1e-3 * rng.standard_normal((spec.S, 3, 3))
+    g, o = pair(spec)
+    for s in range(spec.S):
+        ref = o.field_terms(s, terms=oc.T_DMI)[oc.T_DMI]
+        plain = oc_interfacial_only(o, s)
+        assert field_err(plain, ref) > 1e-2                     # the tensor part matters here
+        assert field_err(g.eval_heff(s, mmx.T_DMI), ref) < FIELD_TOL, (name, s)
+        assert field_err(g.eval_heff(s, mmx.T_ALL), o.heff(s)) < FIELD_TOL, (name, s)
+        assert field_err(g.eval_torque(s), o.torque(s)) < FIELD_TOL, (name, s)
+    Eg, Eo = g.energy(mmx.T_DMI), o.energy(oc.T_DMI)
+    assert abs(Eg - Eo) < 1e-5 * abs(Eo)
+    dt = spec.integrator["dt"]
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=20)
+    o.step_dp45_fixed(dt, 20)
+    for s in range(spec.S):
+        assert np.abs(g.get_state(mmx.F_M0 + s).astype(np.float64) - o.m[s]).max() <= 1e-4
+    g.destroy()
+
+
+def oc_interfacial_only(o, s):
+    from oracle import fields as fl
+    return fl.dmi_interfacial(o.m[s], o.p[s]["Ms"], o.p[s]["D"], o.cell, o.pbc)
