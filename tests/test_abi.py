@@ -58,6 +58,13 @@ def test_argument_errors(lib):
     assert rc == -1
     assert lib.mmx_world_destroy(None) == 0
     assert lib.mmx_step_rk4(None, 1e-13, 1) == -1
+    # entry points added after the first path: NULL world is an argument error, never a crash
+    q9 = (ctypes.c_double * 9)()
+    n = ctypes.c_longlong()
+    assert lib.mmx_set_dmi_tensor(None, 0, q9) == -1
+    assert lib.mmx_graph_enable(None, 1) == -1
+    assert lib.mmx_graph_info(None, ctypes.byref(n)) == -1
+    assert lib.mmx_set_elastic(None, None) == -1 and lib.mmx_set_coupling(None, None) == -1
 
 
 @pytest.mark.parametrize("grid,cell,pbc", [((8, 8, 4), (4e-9, 4e-9, 4e-9), (0, 0, 0)),

@@ -228,3 +228,34 @@ def test_c4_full_size_invariants_of_the_trajectory():
         trapezoid = 0.5 * (P[-2] + P[-1]) * n * dt
         assert abs(lost - trapezoid) < 0.02 * lost, (lost, trapezoid)
     g.destroy()
+
+
+def test_every_setter_invalidates_the_step_graph():
+    """Kernel arguments are baked into the captured graph: each configuration call must make the next
+    stepping call rebuild it (and a cleared DMI tensor must give the plain result again)."""
+    spec = wl.make("c2", (32, 32, 1))
+    dt = spec.integrator["dt"]
+    g = mmx.World.from_spec(spec)
+    ref = mmx.World.from_spec(spec)
+    ref.graph_enable(False)
+
+    def step_both():
+        for w in (g, ref):
+            w.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=3)
+        assert g.graph_info() > 0
+        assert np.array_equal(g.get_state(mmx.F_M0), ref.get_state(mmx.F_M0))
+
+    step_both()
+    q = 1e-3 * np.arange(9, dtype=np.float64).reshape(3, 3)
+    changes = [lambda w: w.set_bext((0.0, 0.2, -0.1)),
+               lambda w: w.set_current((1e11, 0.0, 0.0)),
+               lambda w: w.set_dmi_tensor(0, q),
+               lambda w: w.set_dmi_tensor(0, None),
+               lambda w: w.enable_demag(False),
+               lambda w: w.enable_demag(True)]
+    for change in changes:
+        for w in (g, ref):
+            change(w)
+        assert g.graph_info() == 0
+        step_both()
+    g.destroy(); ref.destroy()
