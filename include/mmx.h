@@ -211,7 +211,10 @@ int mmx_kernel_spectrum_host(const int grid[3], const double cellsize[3], const 
 
 /* ---- evaluation ------------------------------------------------------------------------ */
 
-/* Effective field of one sublattice, restricted to term_mask, of the current state (T). */
+/* Effective field of one sublattice, restricted to term_mask, of the current state (T).
+ * out: fp32 [3][Nz][Ny][Nx].  Cells without a magnet (Ms = 0 for this sublattice) report 0 for every
+ * term, the magnetostatic one included: B_eff is the field acting on m, the stray field in empty
+ * cells is not part of this call.  mmx_eval_torque likewise reports 0 there. */
 int mmx_eval_heff(mmx_world* w, int sublattice, unsigned term_mask, float* out, int mem);
 /* Torque dm/dt (Eq.1-2 + Zhang-Li) of one sublattice for the current state (1/s), all
  * enabled terms. */
