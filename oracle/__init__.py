@@ -14,8 +14,10 @@ Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline /
 Pin status (see tests/test_oracle_*.py and DESIGN.md section "Oracle pins"):
   newell / demag .......... pinned (P1-P5, P19, mpmath spot values, dipole limit)
   exchange, DMI, anisotropy pinned (P6, P10, P11; general DMI tensor of Eq.4: P22)
-  sublattice exchange ..... pinned (P10, P12); homogeneous DMI Eq.6 pinned (P21)
-  LLG torque, integrators . pinned (P7, P8, P9, P14)
+  sublattice exchange ..... pinned (A12 term: P6b two-sublattice spin waves, factor and partner wiring;
+                            A0 term: P12); homogeneous DMI Eq.6 pinned (P21)
+  LLG torque, integrators . pinned (P7, P8, P9; P14: rooted-tree order conditions of RK4 and of all five
+                            embedded pairs of Table 2, observed orders, estimate scaling)
   Zhang-Li torque ......... pinned (P13: Gilbert-form identity, rigid translation at -u)
   elastic / magnetoelastic  pinned (P15 paper numbers, P16 patch test, P17; viscous term P20 paper numbers)
   adaptive-step controller constants (S21), PBC image window (S13), which

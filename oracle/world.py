@@ -51,6 +51,7 @@ class World:
         self._octant = None
         self._spectrum = None
         self._k1 = None
+        self._k1_tab = None
         self.V = self.cell[0] * self.cell[1] * self.cell[2]
 
     # ------------------------------------------------------------------ demag
@@ -193,25 +194,34 @@ class World:
             self.set_state(y)
             self.t += dt
 
-    def step_dp45_fixed(self, dt, nsteps=1):
-        """Forced-accept DP45 steps; returns the list of error estimates (S29 protocol)."""
+    def step_embedded_fixed(self, dt, nsteps=1, tab=rk.DP45):
+        """Forced-accept steps of an embedded pair of Table 2; returns the list of error
+        estimates dt max_c |sum_j e_j k_j|_2 (S29 protocol).  FSAL pairs reuse k_last as the next k_1."""
         errs = []
         for _ in range(nsteps):
-            y, ks, err = rk.rk_step(self.rhs, self.project, self.get_state(), self.t, dt, rk.DP45, self._k1)
+            k1 = self._k1 if (tab.fsal and self._k1_tab is tab) else None
+            y, ks, err = rk.rk_step(self.rhs, self.project, self.get_state(), self.t, dt, tab, k1)
             self.set_state(y)
-            self._k1 = ks[-1]
+            if tab.fsal:
+                self._k1, self._k1_tab = ks[-1], tab
             self.t += dt
             errs.append(self.mag_norm(err))
         return errs
+
+    def step_dp45_fixed(self, dt, nsteps=1):
+        return self.step_embedded_fixed(dt, nsteps, rk.DP45)
 
     def max_torque(self):
         k = self.rhs(self.get_state(), self.t)
         return self.mag_norm(k)
 
-    def run_dp45(self, tol=1e-5, dt0=None, nsteps=None, t_end=None, max_attempts=100000):
-        """Adaptive DP45 (controller S21).  Returns dict(accepted, rejected, dt, t, last_err)."""
-        if self._k1 is None:
-            self._k1 = self.rhs(self.get_state(), self.t)
+    def run_adaptive(self, tab=rk.DP45, tol=1e-5, dt0=None, nsteps=None, t_end=None, max_attempts=100000,
+                     log=None):
+        """Adaptive stepping with an embedded pair (controller S21; the step-size exponent is
+        1/convergence order).  Returns dict(accepted, rejected, dt, t, last_err); `log`, when a list,
+        receives one (dt, err, accepted) tuple per attempt."""
+        if self._k1 is None or self._k1_tab is not tab:
+            self._k1, self._k1_tab = self.rhs(self.get_state(), self.t), tab
         dt = dt0 if dt0 else 0.01 / self.mag_norm(self._k1)
         acc = rej = 0
         last = 0.0
@@ -220,18 +230,26 @@ class World:
                 break
             if t_end is not None and self.t >= t_end:
                 break
-            y, ks, err = rk.rk_step(self.rhs, self.project, self.get_state(), self.t, dt, rk.DP45, self._k1)
+            if t_end is not None and self.t + dt > t_end:
+                dt = t_end - self.t
+            y, ks, err = rk.rk_step(self.rhs, self.project, self.get_state(), self.t, dt, tab, self._k1)
             last = self.mag_norm(err)
-            ok, dt_new = rk.controller(dt, last, tol)
+            ok, dt_new = rk.controller(dt, last, tol, tab.order)
+            if log is not None:
+                log.append((dt, last, bool(ok)))
             if ok:
                 self.set_state(y)
-                self._k1 = ks[-1]
+                self._k1 = ks[-1] if tab.fsal else self.rhs(self.get_state(), self.t + dt)
+                self._k1_tab = tab
                 self.t += dt
                 acc += 1
             else:
                 rej += 1
             dt = dt_new
         return dict(accepted=acc, rejected=rej, dt=dt, t=self.t, last_err=last)
+
+    def run_dp45(self, tol=1e-5, dt0=None, nsteps=None, t_end=None, max_attempts=100000, log=None):
+        return self.run_adaptive(rk.DP45, tol, dt0, nsteps, t_end, max_attempts, log)
 
     # ------------------------------------------------------------------ energies (step 11, S28)
     def energy(self, terms=T_ALL):

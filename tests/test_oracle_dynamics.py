@@ -36,32 +36,64 @@ def test_P7_macrospin_precession_and_damping():
         assert abs(np.linalg.norm(w.m[0].ravel()) - 1) < 1e-15  # P8
 
 
+def _order_conditions(a, c, order):
+    """Rooted-tree order conditions of an explicit Runge-Kutta method up to `order` <= 5 (Butcher):
+    list of (elementary-weight vector Phi, 1/gamma); weights b reach the order iff b.Phi = 1/gamma."""
+    one = np.ones_like(c)
+    Ac = a @ c
+    trees = {1: [(one, 1.0)],
+             2: [(c, 1 / 2)],
+             3: [(c ** 2, 1 / 3), (Ac, 1 / 6)],
+             4: [(c ** 3, 1 / 4), (c * Ac, 1 / 8), (a @ c ** 2, 1 / 12), (a @ Ac, 1 / 24)],
+             5: [(c ** 4, 1 / 5), (c ** 2 * Ac, 1 / 10), (c * (a @ c ** 2), 1 / 15), (c * (a @ Ac), 1 / 30),
+                 (Ac * Ac, 1 / 20), (a @ c ** 3, 1 / 20), (a @ (c * Ac), 1 / 40), (a @ (a @ c ** 2), 1 / 60),
+                 (a @ (a @ Ac), 1 / 120)]}
+    return [t for p in range(1, order + 1) for t in trees[p]]
+
+
+def _residual(tab_a, c, wts, order):
+    return max(abs(float(wts @ phi) - g) for phi, g in _order_conditions(tab_a, c, order))
+
+
 def test_P14_tableau_identities():
-    for tab in (rk.RK4, rk.DP45):
-        assert abs(sum(tab.b) - 1) < 1e-15
-        for i in range(tab.stages):
-            assert abs(sum(tab.a[i]) - tab.c[i]) < 1e-15
+    """Every pair of Table 2 + RK4: row sums, sum b = sum b* = 1, and the rooted-tree
+    order conditions: the propagated weights b satisfy all conditions up to the convergence order
+    the table prints and NOT the next order; the embedded weights b* = b - e those up to the
+    error-estimate order it prints, and not the next.  A wrong sign, a swapped entry or a dropped
+    term in any a_ij, b_j or e_j fails one of these."""
+    cases = [(rk.RK4, 4, None), (rk.HEUN12, 2, 1), (rk.BS23, 3, 2), (rk.CK45, 5, 4), (rk.RKF45, 5, 4), (rk.DP45, 5, 4)]
+    for tab, p, pe in cases:
+        s = tab.stages
+        a = np.zeros((s, s))
+        for i, row in enumerate(tab.a):
+            a[i, :len(row)] = row
+        c = np.array(tab.c)
+        b = np.array(tab.b)
+        assert tab.order == p
+        assert abs(b.sum() - 1) < 1e-15
+        np.testing.assert_allclose(a.sum(axis=1), c, atol=1e-15)
+        assert np.all(np.triu(a) == 0)                      # explicit
+        assert _residual(a, c, b, p) < 1e-14, tab
+        if p < 5:
+            assert _residual(a, c, b, p + 1) > 1e-3, tab    # and not more
+        if pe is None:
+            assert tab.e is None
+            continue
+        bs = b - np.array(tab.e)
+        assert abs(bs.sum() - 1) < 1e-15
+        assert _residual(a, c, bs, pe) < 1e-14, tab
+        assert _residual(a, c, bs, pe + 1) > 1e-4, tab
+        if tab.fsal:                                         # last row of a equals b
+            np.testing.assert_allclose(a[s - 1, :s - 1], b[:s - 1], atol=0)
+            assert b[s - 1] == 0
     # e = b - b*, b* the embedded 4th-order weights of the Dormand-Prince pair (ref [55])
     bstar = [Fr(5179, 57600), 0, Fr(7571, 16695), Fr(393, 640), Fr(-92097, 339200), Fr(187, 2100), Fr(1, 40)]
-    for bj, bs, ej in zip(rk.DP45.b, bstar, rk.DP45.e):
-        assert abs((bj - float(bs)) - ej) < 1e-16
-    # order conditions: b up to order 5 (bushy + a few tall trees), b* up to order 4
-    a = np.zeros((7, 7))
-    for i, row in enumerate(rk.DP45.a):
-        a[i, :len(row)] = row
-    c = np.array(rk.DP45.c)
-    for wts, order in ((np.array(rk.DP45.b), 5), (np.array([float(x) for x in bstar]), 4)):
-        for k in range(order):
-            assert abs(wts @ c ** k - 1 / (k + 1)) < 1e-14
-        assert abs(wts @ (a @ c) - 1 / 6) < 1e-14
-        assert abs(wts @ (a @ c ** 2) - 1 / 12) < 1e-14
-        assert abs(wts @ (a @ (a @ c)) - 1 / 24) < 1e-14
-        assert abs(wts @ (c * (a @ c)) - 1 / 8) < 1e-14
-    b5 = np.array(rk.DP45.b)
-    assert abs(b5 @ (a @ c ** 3) - 1 / 20) < 1e-14
-    assert abs(b5 @ (a @ (a @ (a @ c))) - 1 / 120) < 1e-14
-    # FSAL: last row of a equals b
-    np.testing.assert_allclose(rk.DP45.a[6], rk.DP45.b[:6])
+    for bj, bs_, ej in zip(rk.DP45.b, bstar, rk.DP45.e):
+        assert abs((bj - float(bs_)) - ej) < 1e-16
+    assert rk.EMBEDDED["ck45"][0] is rk.CK45 and rk.EMBEDDED["ck45"][1] == 4
+
+
+TABLEAUX = {"rk4": rk.RK4, "heun12": rk.HEUN12, "bs23": rk.BS23, "ck45": rk.CK45, "rkf45": rk.RKF45, "dp45": rk.DP45}
 
 
 def _final_error(method, dt, T=2e-11, alpha=0.3):
@@ -70,22 +102,42 @@ def _final_error(method, dt, T=2e-11, alpha=0.3):
     if method == "rk4":
         w.step_rk4(dt, n)
     else:
-        w.step_dp45_fixed(dt, n)
+        w.step_embedded_fixed(dt, n, TABLEAUX[method])
     return np.abs(w.m[0].ravel() - _macrospin_exact(alpha, 2.0, (0.6, 0.0, 0.8), n * dt)).max()
 
 
 def test_P14_observed_orders():
-    """Table 2: Dormand-Prince convergence order 5, error-estimate order 4; RK4 order 4."""
-    e1, e2 = _final_error("rk4", 1e-12), _final_error("rk4", 0.5e-12)
-    assert 3.7 < np.log2(e1 / e2) < 4.4
-    e1, e2 = _final_error("dp45", 1e-12), _final_error("dp45", 0.5e-12)
-    assert 4.6 < np.log2(e1 / e2) < 5.5
-    # local error estimate ~ dt^5 (a 4th-order embedded solution)
-    est = []
-    for dt in (1e-12, 0.5e-12):
+    """Table 2: observed global convergence order of every method against the closed-form
+    macrospin, and the dt-scaling of the embedded error estimate: a pair whose embedded solution has
+    order q gives an estimate ~ dt^(q+1)."""
+    for method, p, q, dts in (("rk4", 4, None, (1e-12, 0.5e-12)), ("heun12", 2, 1, (2e-13, 1e-13)),
+                              ("bs23", 3, 2, (4e-13, 2e-13)), ("ck45", 5, 4, (1e-12, 0.5e-12)),
+                              ("rkf45", 5, 4, (1e-12, 0.5e-12)), ("dp45", 5, 4, (1e-12, 0.5e-12))):
+        e1, e2 = _final_error(method, dts[0]), _final_error(method, dts[1])
+        assert p - 0.4 < np.log2(e1 / e2) < p + 0.5, (method, np.log2(e1 / e2))
+        if q is None:
+            continue
+        est = []
+        for dt in dts:
+            w = _macrospin(0.3, B=2.0)
+            est.append(w.step_embedded_fixed(dt, 1, TABLEAUX[method])[0])
+        assert q + 0.6 < np.log2(est[0] / est[1]) < q + 1.4, (method, np.log2(est[0] / est[1]))
+
+
+def test_P14_adaptive_run_meets_its_tolerance():
+    """Controller reading S21 on the closed-form macrospin with every embedded pair: the adaptive run
+    lands on t_end exactly, rejects at least once from a far too large first step, and its global
+    error stays within a small multiple of tol (a wrong sign in an e row makes the estimate useless:
+    either no step is ever rejected or the error is orders of magnitude above tol)."""
+    for name in ("heun12", "bs23", "ck45", "rkf45", "dp45"):
         w = _macrospin(0.3, B=2.0)
-        est.append(w.step_dp45_fixed(dt, 1)[0])
-    assert 4.6 < np.log2(est[0] / est[1]) < 5.4
+        tol = 1e-6
+        log = []
+        st = w.run_adaptive(TABLEAUX[name], tol=tol, dt0=2e-11, t_end=2e-11, log=log)
+        assert abs(st["t"] - 2e-11) < 1e-24 and st["rejected"] >= 1, (name, st)
+        err = np.abs(w.m[0].ravel() - _macrospin_exact(0.3, 2.0, (0.6, 0.0, 0.8), 2e-11)).max()
+        assert err < 30 * tol * max(1, st["accepted"] / 10), (name, err, st)
+        assert all(e <= tol for _, e, ok in log if ok) and all(e > tol for _, e, ok in log if not ok)
 
 
 def _small_world(alpha, seed=21, S=1, J=(0, 0, 0)):

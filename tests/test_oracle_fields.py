@@ -22,6 +22,37 @@ def test_P6_exchange_spin_wave():
     np.testing.assert_allclose(B, want, rtol=0, atol=1e-12 * np.abs(want).max())
 
 
+def test_P6b_inter_sublattice_exchange_spin_waves():
+    """Eq.3 second term, through World.field_terms so the sublattice wiring is pinned
+    too: two periodic sublattices carrying spin waves of DIFFERENT wave numbers k1, k2 (and
+    different Ms).  B_A12 on sublattice s must be (A12/Ms_s) lap m^(s') -- the OTHER sublattice's
+    wave, factor 1 (not the 2 of the first term), divided by its OWN Ms:
+        B_A12^(1) = -(A12/Ms1)(2/h^2)(1 - cos k2 h) m2,   B_A12^(2) = -(A12/Ms2)(2/h^2)(1 - cos k1 h) m1.
+    The same world also pins the first term on each sublattice with its own A11, Ms (P6)."""
+    nx, ny, h = 48, 4, 2e-9
+    A12, Ms, A11 = -1.0e-12, (4.0e5, 2.5e5), (1.0e-11, 0.7e-11)
+    ks = [2 * np.pi * q / (nx * h) for q in (3, 5)]
+    x = (np.arange(nx) + 0.5) * h
+    ms = []
+    for k in ks:
+        m = np.zeros((3, 1, ny, nx))
+        m[0], m[1] = np.cos(k * x)[None, None, :], np.sin(k * x)[None, None, :]
+        ms.append(m)
+    spec = wl.WorldSpec(name="sw2", grid=(nx, ny, 1), cell=(h, h, h), pbc=(1, 1, 0), S=2, demag=False,
+                        mat=wl.make_mat(2, Ms=np.array(Ms)[:, None], A=np.array(A11)[:, None]),
+                        coupling=wl.default_coupling(A12=A12), m=[m.astype(np.float32) for m in ms])
+    w = World(spec)
+    w.m = [m.copy() for m in ms]
+    for s in range(2):
+        o = 1 - s
+        got = w.field_terms(s, terms=T_A12)[T_A12]
+        want = -(A12 / Ms[s]) * (2 / h ** 2) * (1 - np.cos(ks[o] * h)) * ms[o]
+        np.testing.assert_allclose(got, want, rtol=0, atol=1e-12 * np.abs(want).max())
+        got = w.field_terms(s, terms=T_EXCH)[T_EXCH]
+        want = -(2 * A11[s] / Ms[s]) * (2 / h ** 2) * (1 - np.cos(ks[s] * h)) * ms[s]
+        np.testing.assert_allclose(got, want, rtol=0, atol=1e-12 * np.abs(want).max())
+
+
 def test_P11_dmi_cycloid_and_continuum():
     """m = (sin kx, 0, cos kx): B_DMI = -(2D/Ms)(sin kh / h) m; 2-D continuum limit
     (2D/Ms)(dx mz, dy mz, -dx mx - dy my) for a smooth texture."""
