@@ -19,8 +19,9 @@
  *     the caller owns every pointer it passes, the library never keeps it
  *     after the call returns.  The world owns all of its device storage.
  *   - all device work is enqueued on the CUDA stream given at creation
- *     (NULL = legacy default stream).  Calls with host out-parameters
- *     synchronise that stream; the others are asynchronous.
+ *     (NULL: the library creates its own blocking stream, see mmx_world_create).
+ *     Calls with host out-parameters and the stepping calls synchronise that
+ *     stream; the others are asynchronous.
  *   - there is no CPU fallback: without a CUDA device mmx_world_create fails
  *     with MMX_ECUDA.
  */
@@ -126,6 +127,8 @@ typedef struct mmx_rk_opts {
   double t_end;        /* stop when t >= t_end (<= 0: no limit)                         */
   double torque_stop;  /* stop when max|tau| < torque_stop [1/s] (<= 0: off)            */
   long long max_attempts; /* hard cap on attempted steps (<= 0: 1000000)                */
+  double dt_max;       /* adaptive stepping never proposes a step above this (<= 0: none,  */
+                       /* except with elastodynamics on, see mmx_step_rk45)              */
 } mmx_rk_opts;
 
 typedef struct mmx_rk_stats {
@@ -133,7 +136,10 @@ typedef struct mmx_rk_stats {
   double t;          /* simulation time after the call                                 */
   double dt;         /* step size proposed for the next step                           */
   double last_err;   /* error estimate of the last attempted step                      */
-  double max_torque; /* max_c |tau_c| [1/s] at the last accepted state (FSAL methods)  */
+  double max_torque; /* max_c |tau_c| [1/s]: at the last accepted state for the FSAL     */
+                     /* methods (DP45, BS23) and whenever the call stopped on            */
+                     /* torque_stop; otherwise (RK4, Heun, CK45, RKF45) at the state     */
+                     /* the last attempted step started from                             */
   long long launches;/* CUDA kernels launched by this call                             */
 } mmx_rk_stats;
 
@@ -232,8 +238,19 @@ int mmx_max_torque(mmx_world* w, double* out);
 
 /* nsteps classical RK4 steps of size dt (BASELINE config 1 protocol). */
 int mmx_step_rk4(mmx_world* w, double dt, long long nsteps);
-/* Embedded Runge-Kutta stepping (Table 2; default Dormand-Prince).  stats may be NULL
- * (then the call is asynchronous when opts->fixed_dt && nsteps > 0). */
+/* Embedded Runge-Kutta stepping (Table 2; default Dormand-Prince).  stats may be NULL.  The call
+ * returns after the device has finished (it reads the controller block back).
+ *   - t_end > 0 and the current time already >= t_end: nothing is done, MMX_OK, accepted = 0.
+ *   - torque_stop: tested on the torque at the accepted state.  FSAL methods have it as the last
+ *     stage of the step; the others (Heun, Cash-Karp, Fehlberg) evaluate it as the first stage of
+ *     the next attempt and abandon that attempt (it counts neither as accepted nor as rejected).
+ *   - the error estimate is taken over the magnetic variables only (the paper leaves adaptive
+ *     stepping of the elastic variables to future work).  With elastodynamics on, adaptive
+ *     stepping therefore clamps the step to dt_max, and dt_max <= 0 then selects
+ *     0.5 min(cellsize) / sqrt(C11 / rho) (half the explicit stability bound of the fastest
+ *     elastic wave), so that a quiet magnet cannot drive dt past the elastic limit.
+ *   - MMX_ENAN: a NaN/Inf reached the error or torque reduction; the attempt is not accepted, the
+ *     accepted state and time are left as they were, stepping stops. */
 int mmx_step_rk45(mmx_world* w, const mmx_rk_opts* opts, mmx_rk_stats* stats);
 /* Error estimates of the most recent attempted steps (newest last); returns the number
  * written through *n_out (at most n). */

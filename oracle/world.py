@@ -216,16 +216,20 @@ class World:
         return self.mag_norm(k)
 
     def run_adaptive(self, tab=rk.DP45, tol=1e-5, dt0=None, nsteps=None, t_end=None, max_attempts=100000,
-                     log=None):
+                     log=None, dt_max=None):
         """Adaptive stepping with an embedded pair (controller S21; the step-size exponent is
         1/convergence order).  Returns dict(accepted, rejected, dt, t, last_err); `log`, when a list,
-        receives one (dt, err, accepted) tuple per attempt."""
+        receives one (dt, err, accepted) tuple per attempt.  dt_max: no step above it is proposed
+        or taken (the error norm covers the magnetic variables only, S22; with elastodynamics the
+        caller bounds dt by the elastic stability limit)."""
         if self._k1 is None or self._k1_tab is not tab:
             self._k1, self._k1_tab = self.rhs(self.get_state(), self.t), tab
         dt = dt0 if dt0 else 0.01 / self.mag_norm(self._k1)
         acc = rej = 0
         last = 0.0
         for _ in range(max_attempts):
+            if dt_max is not None:
+                dt = min(dt, dt_max)
             if nsteps is not None and acc >= nsteps:
                 break
             if t_end is not None and self.t >= t_end:

@@ -53,7 +53,7 @@ class Elastic(C.Structure):
 class RkOpts(C.Structure):
     _fields_ = [("method", C.c_int), ("fixed_dt", C.c_int), ("dt0", C.c_double), ("tol", C.c_double),
                 ("nsteps", C.c_longlong), ("t_end", C.c_double), ("torque_stop", C.c_double),
-                ("max_attempts", C.c_longlong)]
+                ("max_attempts", C.c_longlong), ("dt_max", C.c_double)]
 
 
 class RkStats(C.Structure):
@@ -317,9 +317,9 @@ class World:
         _check(self.lib.mmx_step_rk4(self.h, float(dt), int(nsteps)))
 
     def step_rk45(self, method=DP45, fixed_dt=False, dt0=0.0, tol=1e-5, nsteps=0, t_end=0.0,
-                  torque_stop=0.0, max_attempts=0):
+                  torque_stop=0.0, max_attempts=0, dt_max=0.0):
         o = RkOpts(int(method), 1 if fixed_dt else 0, float(dt0), float(tol), int(nsteps), float(t_end),
-                   float(torque_stop), int(max_attempts))
+                   float(torque_stop), int(max_attempts), float(dt_max))
         st = RkStats()
         _check(self.lib.mmx_step_rk45(self.h, C.byref(o), C.byref(st)))
         return {k: getattr(st, k) for k, _ in RkStats._fields_}

@@ -334,7 +334,23 @@ int run_steps(mmx_world* w, const mmx_rk_opts* o, mmx_rk_stats* stats) {
 
   MmxCtrl h;
   if (int rc = read_ctrl(w, &h)) return rc;
+  if (o->t_end > 0 && h.t >= o->t_end) {  // already there: no zero or backward step
+    if (stats) {
+      stats->accepted = stats->rejected = 0;
+      stats->t = h.t; stats->dt = o->dt0 > 0 ? o->dt0 : h.dt; stats->last_err = 0.0; stats->max_torque = h.max_torque;
+      stats->launches = 0;
+    }
+    return MMX_OK;
+  }
   h.dt = o->dt0 > 0 ? o->dt0 : 0.0;
+  h.dt_max = o->dt_max > 0 ? o->dt_max : 0.0;
+  if (w->has_elastic && !o->fixed_dt && !(h.dt_max > 0)) {
+    // the error estimate covers the magnetic variables only: keep dt inside the elastic limit
+    double hmin = 1e300;
+    for (int a = 0; a < 3; ++a)
+      if (w->grid[a] > 1 && w->cell[a] < hmin) hmin = w->cell[a];
+    if (hmin < 1e300 && w->el.C11 > 0) h.dt_max = 0.5 * hmin / sqrt(w->el.C11 / w->el.rho);
+  }
   h.tol = o->tol > 0 ? o->tol : 1e-5;
   h.t_end = o->t_end > 0 ? o->t_end : 0.0;
   h.torque_stop = o->torque_stop > 0 ? o->torque_stop : 0.0;

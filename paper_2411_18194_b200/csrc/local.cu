@@ -607,6 +607,7 @@ __global__ void k_controller(MmxCtrl* c, MmxTableau tab, int mode) {
     if (c->dt <= 0.0) {
       const double tq = (double)__uint_as_float(c->tq_bits);
       c->dt = tq > 0.0 ? 0.01 / tq : 1e-15;
+      if (c->dt_max > 0.0 && c->dt > c->dt_max) c->dt = c->dt_max;
     }
     c->max_torque = (double)__uint_as_float(c->tq_bits);
     return;
@@ -614,6 +615,7 @@ __global__ void k_controller(MmxCtrl* c, MmxTableau tab, int mode) {
   if (!c->active) return;
   if (mode == 0) {
     double dt = c->dt;
+    if (!c->fixed && c->dt_max > 0.0 && dt > c->dt_max) dt = c->dt_max;
     if (c->t_end > 0.0 && c->t + dt > c->t_end) dt = c->t_end - c->t;
     c->dt = dt;
     for (int i = 0; i < MMX_MAX_STAGES; ++i) {
@@ -635,6 +637,15 @@ __global__ void k_controller(MmxCtrl* c, MmxTableau tab, int mode) {
   c->attempts++;
   bool accept = c->fixed || !tab.embedded || err <= c->tol;
   if (bad) { c->nan_flag = 1; c->active = 0; accept = false; }
+  // methods without a reusable last stage: stage 0 of this attempt measured the torque of the accepted
+  // state it started from; below torque_stop the attempt is abandoned (neither accepted nor rejected)
+  if (!bad && !tab.fsal && c->torque_stop > 0.0 && (double)__uint_as_float(tb) < c->torque_stop) {
+    c->max_torque = (double)__uint_as_float(tb);
+    c->attempts--;
+    c->hist_n--;
+    c->active = 0;
+    return;
+  }
   double dt_new = c->dt;
   if (!c->fixed && tab.embedded) {
     double fac = 2.0;
@@ -643,6 +654,7 @@ __global__ void k_controller(MmxCtrl* c, MmxTableau tab, int mode) {
       fac = fmin(2.0, fmax(0.5, fac));
     }
     dt_new = c->dt * 0.8 * fac;
+    if (c->dt_max > 0.0 && dt_new > c->dt_max) dt_new = c->dt_max;
   }
   if (accept) {
     c->t += c->dt;

@@ -28,7 +28,7 @@ enum {
 struct MmxCtrl {
   double t, dt, tol;
   double err_last, max_torque;
-  double t_end, torque_stop;
+  double t_end, torque_stop, dt_max;
   long long accepted, rejected, attempts, target_accepted;
   int sel;       // which of the two state buffers holds the accepted state
   int active;    // 0: all kernels of further attempts are no-ops

@@ -21,6 +21,20 @@ def field_err(got, ref):
     return float((d / np.maximum(n, 0.1 * rms)).max())
 
 
+def torque_err_conditioned(got, ref, B, alpha, gamma):
+    """Torque parity for states near equilibrium.  There tau = -gamma' [m x B +
+    alpha m x (m x B)] is a small remainder of a large field nearly parallel to m (33 T of
+    inter-sublattice exchange in c3 / c5), so an admissible field error of FIELD_TOL |B| already moves
+    the torque by gamma' (1 + alpha) FIELD_TOL |B| -- far more than FIELD_TOL |tau|.  The criterion is
+    the north_star field tolerance propagated through Eq.2:
+        max_c |d tau_c| / (gamma' (1 + alpha) max(|B_c|, 0.1 RMS|B|)),   gamma' = gamma / (1 + alpha^2)."""
+    d = np.sqrt(((np.asarray(got, np.float64) - ref) ** 2).sum(axis=0))
+    n = np.sqrt((np.asarray(B, np.float64) ** 2).sum(axis=0))
+    rms = np.sqrt((n ** 2).mean())
+    scale = gamma / (1 + alpha ** 2) * (1 + alpha) * np.maximum(n, 0.1 * rms)
+    return float((d / scale).max())
+
+
 def max_dm(a, b):
     return float(np.abs(np.asarray(a, np.float64) - np.asarray(b, np.float64)).max())
 
@@ -33,6 +47,11 @@ def pair(spec, demag_mode="fft", demag=None):
     g = mmx.World.from_spec(spec)
     o = OracleWorld(spec, demag_mode=demag_mode)
     return g, o
+
+
+def pair_oracle(spec, demag_mode="fft"):
+    """A fresh oracle world alone (no CUDA world)."""
+    return OracleWorld(spec, demag_mode=demag_mode)
 
 
 def gpu_m(g, S):

@@ -36,7 +36,7 @@ def test_every_declared_symbol_is_exported(lib):
 def test_struct_layouts_match_header():
     assert ctypes.sizeof(binding.Material) == 20 * 8
     assert ctypes.sizeof(binding.Coupling) == 9 * 8
-    assert ctypes.sizeof(binding.RkOpts) == 56 and ctypes.sizeof(binding.RkStats) == 56
+    assert ctypes.sizeof(binding.RkOpts) == 64 and ctypes.sizeof(binding.RkStats) == 56
     assert ctypes.sizeof(binding.Elastic) == 88
 
 

@@ -6,7 +6,7 @@ import pytest
 
 import paper_2411_18194_b200 as mmx
 import workloads as wl
-from gpu_util import TRAJ_TOL, gpu_m, max_dm, pair
+from gpu_util import TRAJ_TOL, gpu_m, max_dm, pair, pair_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -80,16 +80,95 @@ def test_split_calls_equal_one_call():
 
 
 def test_adaptive_controller_matches_oracle():
-    """Adaptive DP45 (controller reading S21): same accept/reject sequence and step sizes."""
+    """Adaptive DP45 (controller reading S21) from a first step 60x the one the controller settles on:
+    both sides reject several times, shrink and recover; every attempt must take the same accept /
+    reject decision with the same step size and estimate (per-attempt calls, max_attempts = 1, the
+    proposed dt handed back in), then a free-running stretch must end at the same time and state."""
     spec = wl.make("c2", (32, 32, 1))
     g, o = pair(spec)
-    n = 40
-    st = g.step_rk45(method=mmx.DP45, tol=1e-5, nsteps=n)
-    ref = o.run_dp45(tol=1e-5, nsteps=n)
-    assert st["accepted"] == n == ref["accepted"]
-    assert abs(st["rejected"] - ref["rejected"]) <= 1
-    assert abs(st["t"] - ref["t"]) <= 2e-3 * ref["t"]
-    _compare_state(g, o, spec, tol=5e-4)
+    tol = 1e-5
+    settle = o.run_dp45(tol=tol, nsteps=12)["dt"]
+    o = pair_oracle(spec)
+    log = []
+    o.run_dp45(tol=tol, dt0=60 * settle, max_attempts=16, log=log)
+    nrej = sum(1 for _, _, ok in log if not ok)
+    assert nrej >= 3 and len(log) - nrej >= 3, log
+    dt = 60 * settle
+    for k, (dt_ref, err_ref, ok_ref) in enumerate(log):
+        st = g.step_rk45(method=mmx.DP45, tol=tol, dt0=dt, max_attempts=1)
+        assert (st["accepted"] == 1) == ok_ref and st["accepted"] + st["rejected"] == 1, (k, st, log[k])
+        assert abs(dt - dt_ref) <= 1e-3 * dt_ref, (k, dt, dt_ref)
+        assert abs(st["last_err"] - err_ref) <= 2e-2 * err_ref + 1e-9, (k, st["last_err"], err_ref)
+        dt = st["dt"]
+    _compare_state(g, o, spec)
+    n = 20
+    st = g.step_rk45(method=mmx.DP45, tol=tol, dt0=dt, nsteps=n)
+    ref = o.run_dp45(tol=tol, dt0=dt, nsteps=n)
+    assert st["accepted"] == n == ref["accepted"] and st["rejected"] == ref["rejected"]
+    assert abs(st["t"] - ref["t"]) <= 1e-4 * ref["t"]
+    # the two sides now stand at slightly different times (their step sizes follow estimates that agree
+    # to ~1e-3): the states may differ by that time offset times the largest |dm/dt|, on top of TRAJ_TOL
+    _compare_state(g, o, spec, tol=TRAJ_TOL + o.max_torque() * abs(st["t"] - ref["t"]))
+    g.destroy()
+
+
+def test_nan_in_the_state_is_reported_and_leaves_the_accepted_state_alone():
+    """MMX_ENAN ("NaN guard"): one NaN cell written through mmx_set_state must
+    surface as status MMX_ENAN from the stepping call, with no step accepted, the time and the
+    state buffer of the accepted side untouched, and max_torque reporting it too."""
+    spec = wl.make("c4", (16, 16, 8))
+    g = mmx.World.from_spec(spec)
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=1e-13, nsteps=3)
+    t0 = g.get_time()
+    m = g.get_state(mmx.F_M0).copy()
+    m[1, 3, 5, 7] = np.nan
+    g.set_state(mmx.F_M0, m)
+    for kw in (dict(fixed_dt=True, dt0=1e-13, nsteps=5), dict(tol=1e-5, nsteps=5), dict(method=mmx.CK45, tol=1e-5, nsteps=5)):
+        with pytest.raises(mmx.MmxError) as ei:
+            g.step_rk45(**kw)
+        assert ei.value.code == -5, ei.value          # MMX_ENAN
+        assert g.get_time() == t0
+        back = g.get_state(mmx.F_M0)
+        assert np.array_equal(back, m, equal_nan=True)
+    with pytest.raises(mmx.MmxError) as ei:
+        g.max_torque()
+    assert ei.value.code == -5
+    # the world is usable again once the state is repaired
+    m[1, 3, 5, 7] = 0.0
+    m /= np.sqrt((m.astype(np.float64) ** 2).sum(axis=0, keepdims=True)).astype(np.float32)
+    g.set_state(mmx.F_M0, m)
+    st = g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=1e-13, nsteps=2)
+    assert st["accepted"] == 2
+    g.destroy()
+
+
+def test_t_end_already_reached_and_elastic_step_clamp():
+    """(a) a stepping call whose t_end is not ahead of the current time does nothing
+    (no zero or backward step, dt untouched); (b) with elastodynamics on, adaptive stepping keeps
+    dt at or below dt_max = 0.5 min(h) / sqrt(C11 / rho) although the magnetic error is ~ 0."""
+    spec = wl.make("c1", (32, 16, 1))
+    g = mmx.World.from_spec(spec)
+    st = g.step_rk45(method=mmx.DP45, tol=1e-5, t_end=1e-12)
+    assert abs(st["t"] - 1e-12) < 1e-24
+    m = g.get_state(mmx.F_M0)
+    st2 = g.step_rk45(method=mmx.DP45, tol=1e-5, t_end=1e-12)
+    assert st2["accepted"] == 0 and st2["rejected"] == 0 and st2["t"] == st["t"]
+    st3 = g.step_rk45(method=mmx.DP45, tol=1e-5, t_end=0.5e-12)
+    assert st3["accepted"] == 0 and st3["t"] == st["t"]
+    assert np.array_equal(g.get_state(mmx.F_M0), m)
+    st4 = g.step_rk45(method=mmx.DP45, tol=1e-5, t_end=1.5e-12)
+    assert st4["accepted"] > 0 and abs(st4["t"] - 1.5e-12) < 1e-24
+    g.destroy()
+    spec = wl.make("c5", (64, 32, 1))
+    spec.demag = False
+    g = mmx.World.from_spec(spec)
+    lim = 0.5 * 2e-9 / np.sqrt(2.5e11 / 6800.0)
+    st = g.step_rk45(method=mmx.DP45, tol=1e-3, dt0=1e-15, nsteps=60)
+    assert st["accepted"] == 60 and st["dt"] <= lim * (1 + 1e-12), (st, lim)
+    u = g.get_state(mmx.F_U)
+    assert np.all(np.isfinite(u)) and np.abs(u).max() < 1e-9      # stable: no CFL blow-up
+    st = g.step_rk45(method=mmx.DP45, tol=1e-3, dt0=1e-15, nsteps=40, dt_max=2e-14)
+    assert st["dt"] <= 2e-14 * (1 + 1e-12)
     g.destroy()
 
 
