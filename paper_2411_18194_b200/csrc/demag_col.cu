@@ -23,15 +23,13 @@
 // 16-column tiles with the halves in one warp but no pipeline (248 us), the cp.async pipeline with
 // the kernel values in registers (207 us; 272 us with 8-column tiles); k_inner_q runs at 170 us.
 // A persistent y pass with register prefetch (89 us) lost to k_mid_pipe (66 / 76 us).
+#ifndef MMX_PACKED_R16
 #define MMX_PACKED_R16 0   // measured on c4: y passes 68.0 / 80.8 us packed, 66.1 / 78.4 us scalar
+#endif
 #include "fft_reg.cuh"
 #include "mmx_internal.h"
 
 using namespace mmxreg;
-
-#ifndef MMX_MID_PIPE
-#define MMX_MID_PIPE 1        // 1: pipelined y pass (cp.async stages) for 512-point lines on large grids
-#endif
 
 namespace {
 
@@ -86,8 +84,6 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_q(InnerColArgs a) {
     twp[q] = h ? a.tw[j + R * q] : make_float2(1.f, 0.f);
   }
 
-  pdl_wait();      // the twiddle loads above do not depend on the previous kernel
-  pdl_trigger();   // persistent kernel: the next kernel's CTAs take over as ours exit
   if (a.gated && !a.ctrl->active) return;
 
   auto tile_ko = [&](int tile) -> int {
@@ -211,9 +207,9 @@ __global__ void __launch_bounds__(32 * R, 2) k_inner_q(InnerColArgs a) {
       const float k4 = __uint_as_float(__float_as_uint(kp[4 * (H + 1) * TL]) ^ mo4 ^ (mir ? mi4 : 0u));
       const float k5 = __uint_as_float(__float_as_uint(kp[5 * (H + 1) * TL]) ^ mo5 ^ (mir ? mi5 : 0u));
       const float2 mx = X[0][b], my = X[1][b], mz = X[2][b];
-      X[0][b] = make_float2(fmaf(k0, mx.x, fmaf(k3, my.x, k4 * mz.x)), fmaf(k0, mx.y, fmaf(k3, my.y, k4 * mz.y)));
-      X[1][b] = make_float2(fmaf(k3, mx.x, fmaf(k1, my.x, k5 * mz.x)), fmaf(k3, mx.y, fmaf(k1, my.y, k5 * mz.y)));
-      X[2][b] = make_float2(fmaf(k4, mx.x, fmaf(k5, my.x, k2 * mz.x)), fmaf(k4, mx.y, fmaf(k5, my.y, k2 * mz.y)));
+      X[0][b] = rfma(k0, mx, rfma(k3, my, rmul(k4, mz)));
+      X[1][b] = rfma(k3, mx, rfma(k1, my, rmul(k5, mz)));
+      X[2][b] = rfma(k4, mx, rfma(k5, my, rmul(k2, mz)));
     }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -353,17 +349,9 @@ __global__ void __launch_bounds__(2 * R * TILE, 2) k_mid_col(MidColArgs a) {
 // (lane = column + 8 h + 16 (j & 1)), the rows of the next tile stream into shared memory with
 // cp.async while the current tile is transformed; the halves of the inverse meet by shuffle.
 // Small CTAs (16 R threads, 65-97 KB) so that three (forward) or two (inverse) of them share an SM.
-#ifndef MMX_MIDP_TW_REGS
-#define MMX_MIDP_TW_REGS 1   // stage twiddles of a thread live in registers for the whole kernel
-#endif
-#ifndef MMX_MIDP_MINB_F
-#define MMX_MIDP_MINB_F 2   // (2 CTAs of 128 registers beat 3 of 80 once the twiddles are register-resident)
-#endif
-#ifndef MMX_MIDP_MINB_I
-#define MMX_MIDP_MINB_I 2
-#endif
+// (two CTAs of 128 registers per SM beat three of 80 once the twiddles are register-resident)
 template <int R, int DIR>
-__global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_MINB_I) k_mid_pipe(MidColArgs a) {
+__global__ void __launch_bounds__(16 * R, 2) k_mid_pipe(MidColArgs a) {
   constexpr int H = R * R, P = 2 * H, TL = 8, NT = 16 * R;
   constexpr int ROWS = DIR < 0 ? H : P;   // rows of a staged tile
   constexpr int EXT = H * TL + 8;         // exchange tile of one half (+8: the halves use different banks)
@@ -377,24 +365,17 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
   const int ntm = a.ntile_main * a.nslab;
   const int nt = ntm + (a.nyq ? (a.nslab + TL - 1) / TL : 0);
   float2* ex = exb + h * EXT + kxl;
-#if MMX_MIDP_TW_REGS
   // stage twiddles w_H^(j q) of this thread, loaded once for all tiles
   float2 tws[R];
 #pragma unroll
   for (int q = 0; q < R; ++q) tws[q] = a.tw[2 * j * q];
-#define MMX_TWS(q) tws[q]
   // forward pass: also the half twiddles w_P^(j + R u) (identity for the even half)
   float2 twp[DIR < 0 ? R : 1];
   if (DIR < 0) {
 #pragma unroll
     for (int u = 0; u < R; ++u) twp[u] = h ? a.tw[j + R * u] : make_float2(1.f, 0.f);
   }
-#else
-#define MMX_TWS(q) stw[2 * j * (q)]
-#endif
 
-  pdl_wait();      // the twiddle loads above do not depend on the previous kernel
-  pdl_trigger();   // persistent kernel: the next kernel's CTAs take over as ours exit
   if (a.gated && !a.ctrl->active) return;
 
   auto issue = [&](int tile, int buf) {
@@ -453,12 +434,7 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
 #pragma unroll
       for (int u = 0; u < R; ++u) {
         const float2 x = xin[(j + R * u) * TL];
-#if MMX_MIDP_TW_REGS
         v[u] = cmul(x, twp[u]);
-#else
-        const float2 w = h ? stw[j + R * u] : make_float2(1.f, 0.f);
-        v[u] = cmul(x, w);
-#endif
       }
     } else {
 #pragma unroll
@@ -467,7 +443,7 @@ __global__ void __launch_bounds__(16 * R, DIR < 0 ? MMX_MIDP_MINB_F : MMX_MIDP_M
     Dft<R, DIR>::run(v);
     ex[(0 * R + j) * TL] = v[0];
 #pragma unroll
-    for (int q = 1; q < R; ++q) ex[(q * R + j) * TL] = ctw<DIR>(v[q], MMX_TWS(q));
+    for (int q = 1; q < R; ++q) ex[(q * R + j) * TL] = ctw<DIR>(v[q], tws[q]);
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < R; ++q) v[q] = ex[(j * R + q) * TL];
@@ -556,7 +532,6 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
   const size_t smem = sizeof(float2) * (dir < 0 ? 2 : 3) * R * R * TILE;
   ProfScope ps(w, dir < 0 ? PK_MID_FWD : PK_MID_INV);
   const int ntiles = a.ntile_main * a.nslab + (a.nyq ? (a.nslab + TILE - 1) / TILE : 0);
-#if MMX_MID_PIPE
   if (R == 16 && ntiles >= 8 * w->sm_count && (size_t)a.nslab * a.out_outer < (1ull << 31) &&
       (size_t)a.nslab * a.in_outer < (1ull << 31)) {
     MidColArgs b = a;
@@ -568,17 +543,16 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
     const size_t sm = sizeof(float2) * (2 * (R * R * TL + 8) + 2 * (dir < 0 ? R * R : 2 * R * R) * TL);
     if (dir < 0) {
       if (int rc = set_smem_col(k_mid_pipe<16, -1>, sm)) return rc;
-      int grid = mmx_persistent_grid(k_mid_pipe<16, -1>, 16 * 16, sm, w->sm_count, MMX_MIDP_MINB_F);
+      int grid = mmx_persistent_grid(k_mid_pipe<16, -1>, 16 * 16, sm, w->sm_count, 2);
       MMX_CUDA(mmx_launch(k_mid_pipe<16, -1>, grid < nt ? grid : nt, 16 * 16, sm, w->stream, b));
     } else {
       if (int rc = set_smem_col(k_mid_pipe<16, +1>, sm)) return rc;
-      int grid = mmx_persistent_grid(k_mid_pipe<16, +1>, 16 * 16, sm, w->sm_count, MMX_MIDP_MINB_I);
+      int grid = mmx_persistent_grid(k_mid_pipe<16, +1>, 16 * 16, sm, w->sm_count, 2);
       MMX_CUDA(mmx_launch(k_mid_pipe<16, +1>, grid < nt ? grid : nt, 16 * 16, sm, w->stream, b));
     }
     MMX_CUDA(cudaGetLastError());
     return MMX_OK;
   }
-#endif
   (void)ntiles;
   if (dir < 0) {
     if (int rc = set_smem_col(k_mid_col<R, TILE, -1>, smem)) return rc;

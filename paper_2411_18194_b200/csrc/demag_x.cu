@@ -35,38 +35,6 @@ __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_grou
 template <int N>
 __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// Forward x pass: -DMMX_X_BULK=1 lets the rows of a pair arrive by one TMA bulk copy per warp
-// (cp.async.bulk + mbarrier, SASS UBLKCP) instead of four cp.async per lane.  Measured on c4: 33.1 us
-// against 33.2 us, parity and bitwise-repeatability tests pass either way.  No gain, and the
-// mbarrier / proxy-fence path cannot be put through racecheck on this pool (compute-sanitizer is
-// closed), so the default stays cp.async.
-#ifndef MMX_X_BULK
-#define MMX_X_BULK 0
-#endif
-// TMA bulk copy global -> shared (1-D, contiguous), completion counted in bytes on an mbarrier
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "MMX_WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra MMX_DONE_%=;\n"
-      "bra MMX_WAIT_%=;\n"
-      "MMX_DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
 struct XWArgs {
   int nx, rows, xp, S, gated;
   size_t N;
@@ -91,48 +59,18 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
   // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
   __shared__ float2 stq[XR * (XR + 1)];
-#if MMX_X_BULK
-  __shared__ __align__(8) unsigned long long mbar[XW];  // one per warp: "my next row pair has landed"
-#endif
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = lane >> 1, h = lane & 1;  // one 64-bit shared-memory wavefront = 8 j x both halves
   float* sin_ = reinterpret_cast<float*>(smraw + wid * xfwd_warp_bytes(S));
   float2* sex = reinterpret_cast<float2*>(sin_ + (size_t)S * 2 * XH);
   for (int q = threadIdx.x; q < XH; q += 32 * XW) stw[q] = a.tw[q];
   for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
-  pdl_wait();      // everything above is independent of the previous kernel
-  pdl_trigger();   // persistent kernel: the next kernel's CTAs may take over the SMs as ours exit
   if (a.gated && !a.ctrl->active) return;
   const float* y = a.ctrl->sel ? a.yin[1] : a.yin[0];  // (no dynamic index into the parameter block)
   const int npair = (a.rows + 1) >> 1;
   const int nwarp = gridDim.x * XW;
   const int chunks = nx >> 1;  // 16-byte chunks of a row pair: 2 nx floats / 4
 
-#if MMX_X_BULK
-  // the rows of a pair are contiguous in memory: one bulk copy (TMA) per sublattice, issued by lane 0,
-  // its byte count armed on the warp's mbarrier; every lane then waits on the barrier's phase
-  auto prefetch = [&](int pair) {
-    if (lane == 0) {
-      const bool full = FULL || 2 * pair + 1 < a.rows;
-      const unsigned bytes = (unsigned)((full ? 2 : 1) * nx * sizeof(float));
-      // the buffer was read through the generic proxy; order those reads before the async-proxy write
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(&mbar[wid], bytes * S);
-      for (int s = 0; s < S; ++s)
-        bulk_g2s(sin_ + s * 2 * XH, y + (size_t)s * 3 * a.N + (size_t)pair * 2 * nx, bytes, &mbar[wid]);
-    }
-  };
-  if (lane == 0) mbar_init(&mbar[wid], 1);
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  __syncthreads();  // stw, stq, mbar
-  (void)chunks;
-  unsigned phase = 0;
-  int pair = blockIdx.x * XW + wid;
-  if (pair < npair) prefetch(pair);
-  for (; pair < npair; pair += nwarp) {
-    mbar_wait(&mbar[wid], phase);
-    phase ^= 1;
-#else
   auto prefetch = [&](int pair) {
     for (int s = 0; s < S; ++s) {
       const float* src = y + (size_t)s * 3 * a.N + (size_t)pair * 2 * nx;
@@ -149,7 +87,6 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   for (; pair < npair; pair += nwarp) {
     cp_wait<0>();
     __syncwarp();
-#endif
     const bool two = FULL || 2 * pair + 1 < a.rows;
     float2 v[XR];
 #pragma unroll
@@ -194,8 +131,8 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
       const int k = lane + 32 * i;
       if (k <= XH) {
         const float2 zk = zs[k], zm = zs[(XP - k) & (XP - 1)];
-        o0[k] = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-        if (two) o1[k] = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
+        o0[k] = rmul(0.5f, cadd(zk, make_float2(zm.x, -zm.y)));
+        if (two) o1[k] = rmul(0.5f, cadd(make_float2(zk.y, -zk.x), make_float2(zm.y, zm.x)));
       }
     }
     __syncwarp();  // zs is rewritten by the next iteration
@@ -220,8 +157,6 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   XInvSmem& sm = reinterpret_cast<XInvSmem*>(smraw)[wid];
   for (int q = threadIdx.x; q < XH; q += 32 * XW) stw[q] = a.tw[q];
   for (int q = threadIdx.x; q < XR * XR; q += 32 * XW) stq[(q / XR) * (XR + 1) + q % XR] = a.tw[2 * (q / XR) * (q % XR)];
-  pdl_wait();      // everything above is independent of the previous kernel
-  pdl_trigger();   // persistent kernel: the next kernel's CTAs may take over the SMs as ours exit
   if (a.gated && !a.ctrl->active) return;
   const int npair = (a.rows + 1) >> 1;
   const int nwarp = gridDim.x * XW;
@@ -252,7 +187,7 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
       const int kk = k <= XH ? k : XP - k;
       const float2 va = A[kk];
       const float2 vb = two ? B[kk] : make_float2(0.f, 0.f);
-      v[u] = k <= XH ? make_float2(va.x - vb.y, va.y + vb.x) : make_float2(va.x + vb.y, vb.x - va.y);
+      v[u] = k <= XH ? cadd(va, make_float2(-vb.y, vb.x)) : cadd(make_float2(va.x, -va.y), make_float2(vb.y, vb.x));
     }
     __syncwarp();
     if (pair + nwarp < npair) prefetch(pair + nwarp);  // overlaps the transform below

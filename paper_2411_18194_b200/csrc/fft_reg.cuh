@@ -21,26 +21,42 @@ namespace mmxreg {
 
 #define MMX_DI __device__ __forceinline__
 
-// Complex add / subtract as ONE packed instruction (add.f32x2 / sub.f32x2, sm_100: SASS FADD2): the
-// butterflies are add-dominated and the kernels are bound by instruction issue, not by the fp32
-// pipes, so halving the instruction count of the adds is a direct win.  Same IEEE result per
-// component as the scalar form.
+// Packed fp32 pairs (PTX add / sub / mul / fma .f32x2, sm_100: SASS FADD2 / FMUL2 / FFMA2).  On sm_100 a
+// scalar FFMA / FADD / FMUL occupies the fp32 pipe of a scheduler for two cycles; the packed forms do
+// two lanes' worth in the same slot, so a complex number (re, im) in one aligned register pair halves
+// both the instruction count and the pipe time of the butterflies.  The SASS operands carry free
+// modifiers -- swap of the halves (.LO_HI), a sign per half (.NP / .PN), scalar broadcast (.F32) --
+// and ptxas folds the mov.b64 {hi, lo} packings below into them, so
+//   complex multiply      a w = a (w.x, w.x) + swap(a) (-w.y, w.y)           FMUL2 + FFMA2
+//   b +- i d                  = b +- (-d.y, d.x)                              one FADD2
+//   real scalar k times a     = (k, k) a                                       one FMUL2 / FFMA2
+// (checked with cuobjdump -sass: no MOV / PRMT is emitted for the packings).  Same IEEE operations per
+// component as the scalar forms, in a different association for the multiplies.
+typedef unsigned long long pk2;
+MMX_DI pk2 pk(float lo, float hi) {
+  pk2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+MMX_DI pk2 pk(float2 a) { return pk(a.x, a.y); }
+MMX_DI float2 up(pk2 v) {
+  float2 r;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+  return r;
+}
+MMX_DI pk2 add2(pk2 a, pk2 b) { pk2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+MMX_DI pk2 sub2(pk2 a, pk2 b) { pk2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+MMX_DI pk2 mul2(pk2 a, pk2 b) { pk2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+MMX_DI pk2 fma2(pk2 a, pk2 b, pk2 c) { pk2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+
 #ifndef MMX_PACKED_F32X2
 #define MMX_PACKED_F32X2 1
 #endif
 #ifndef MMX_PACKED_R16
-#define MMX_PACKED_R16 MMX_PACKED_F32X2   // the radix-16 butterflies of the y passes run better on scalar adds
+#define MMX_PACKED_R16 MMX_PACKED_F32X2
 #endif
-MMX_DI float2 cadd_pk(float2 a, float2 b) {
-  unsigned long long ua = *reinterpret_cast<unsigned long long*>(&a), ub = *reinterpret_cast<unsigned long long*>(&b), ud;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(ud) : "l"(ua), "l"(ub));
-  return *reinterpret_cast<float2*>(&ud);
-}
-MMX_DI float2 csub_pk(float2 a, float2 b) {
-  unsigned long long ua = *reinterpret_cast<unsigned long long*>(&a), ub = *reinterpret_cast<unsigned long long*>(&b), ud;
-  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(ud) : "l"(ua), "l"(ub));
-  return *reinterpret_cast<float2*>(&ud);
-}
+MMX_DI float2 cadd_pk(float2 a, float2 b) { return up(add2(pk(a), pk(b))); }
+MMX_DI float2 csub_pk(float2 a, float2 b) { return up(sub2(pk(a), pk(b))); }
 MMX_DI float2 cadd_sc(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 MMX_DI float2 csub_sc(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 template <bool PK>
@@ -49,13 +65,23 @@ template <bool PK>
 MMX_DI float2 csubt(float2 a, float2 b) { return PK ? csub_pk(a, b) : csub_sc(a, b); }
 MMX_DI float2 cadd(float2 a, float2 b) { return caddt<MMX_PACKED_F32X2 != 0>(a, b); }
 MMX_DI float2 csub(float2 a, float2 b) { return csubt<MMX_PACKED_F32X2 != 0>(a, b); }
+#if MMX_PACKED_F32X2
+MMX_DI float2 cmul(float2 a, float2 b) { return up(fma2(pk(a.y, a.x), pk(-b.y, b.y), mul2(pk(a), pk(b.x, b.x)))); }
+// a * conj(b)
+MMX_DI float2 cmulc(float2 a, float2 b) { return up(fma2(pk(a.y, a.x), pk(b.y, -b.y), mul2(pk(a), pk(b.x, b.x)))); }
+// real scalar times complex, and its accumulate form
+MMX_DI float2 rmul(float k, float2 a) { return up(mul2(pk(k, k), pk(a))); }
+MMX_DI float2 rfma(float k, float2 a, float2 c) { return up(fma2(pk(k, k), pk(a), pk(c))); }
+#else
 MMX_DI float2 cmul(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
-// a * conj(b)
 MMX_DI float2 cmulc(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, a.y * b.y), fmaf(a.y, b.x, -a.x * b.y));
 }
+MMX_DI float2 rmul(float k, float2 a) { return make_float2(k * a.x, k * a.y); }
+MMX_DI float2 rfma(float k, float2 a, float2 c) { return make_float2(fmaf(k, a.x, c.x), fmaf(k, a.y, c.y)); }
+#endif
 // a * w (DIR < 0, forward) or a * conj(w) (DIR > 0, inverse), w a forward twiddle
 template <int DIR>
 MMX_DI float2 ctw(float2 a, float2 w) {
@@ -70,16 +96,22 @@ MMX_DI float2 mul_i(float2 a) {
 template <int DIR>
 MMX_DI float2 rot(float2 a, float c, float s) {
   const float d = DIR < 0 ? -s : s;
+#if MMX_PACKED_F32X2
+  return up(fma2(pk(a.y, a.x), pk(-d, d), mul2(pk(a), pk(c, c))));
+#else
   return make_float2(fmaf(a.x, c, -a.y * d), fmaf(a.x, d, a.y * c));
+#endif
 }
 
-// b + (DIR i) d and b - (DIR i) d, scalar (the swap of d's components would cost moves in packed form)
-template <int DIR>
+// b + (DIR i) d and b - (DIR i) d
+template <int DIR, bool PK = (MMX_PACKED_F32X2 != 0)>
 MMX_DI float2 cadd_i(float2 b, float2 d) {
+  if (PK) return DIR < 0 ? up(add2(pk(b), pk(d.y, -d.x))) : up(add2(pk(b), pk(-d.y, d.x)));
   return DIR < 0 ? make_float2(b.x + d.y, b.y - d.x) : make_float2(b.x - d.y, b.y + d.x);
 }
-template <int DIR>
+template <int DIR, bool PK = (MMX_PACKED_F32X2 != 0)>
 MMX_DI float2 csub_i(float2 b, float2 d) {
+  if (PK) return DIR < 0 ? up(sub2(pk(b), pk(d.y, -d.x))) : up(sub2(pk(b), pk(-d.y, d.x)));
   return DIR < 0 ? make_float2(b.x - d.y, b.y + d.x) : make_float2(b.x + d.y, b.y - d.x);
 }
 
@@ -88,9 +120,9 @@ MMX_DI void dft4(float2& x0, float2& x1, float2& x2, float2& x3) {
   const float2 a = caddt<PK>(x0, x2), b = csubt<PK>(x0, x2);
   const float2 c = caddt<PK>(x1, x3), d = csubt<PK>(x1, x3);
   x0 = caddt<PK>(a, c);
-  x1 = cadd_i<DIR>(b, d);
+  x1 = cadd_i<DIR, PK>(b, d);
   x2 = csubt<PK>(a, c);
-  x3 = csub_i<DIR>(b, d);
+  x3 = csub_i<DIR, PK>(b, d);
 }
 
 // X[q] = sum_r v[r] exp(DIR 2 pi i q r / R), natural order in and out

@@ -278,59 +278,29 @@ __device__ __forceinline__ void stq(float* p, size_t N, size_t i, const Q3& q) {
   *reinterpret_cast<float4*>(p + 2 * N + i) = make_float4(q.c[0].z, q.c[1].z, q.c[2].z, q.c[3].z);
 }
 
-#ifndef MMX_L4_MINB
-#define MMX_L4_MINB 2
-#endif
 // NP = n_prev, the number of earlier k_j of the RK combination; MODE bit 0: form the next stage
 // state, bit 1: form the embedded error
-// L2 evict-first hints on the streamed inputs and the k_i stores.  Measured on c4: 2.7026 ms per step
-// with, 2.7070 ms without (0.16 %, inside the scatter between identical builds), and the x forward
-// pass that would profit from a retained y_next did not move (33.2 us both ways): no effect, off.
-#ifndef MMX_L4_EVICT
-#define MMX_L4_EVICT 0
-#endif
-#ifndef MMX_L4_BLOCK
-#define MMX_L4_BLOCK 256
-#endif
+#define MMX_L4_BLOCK 256   // threads per CTA, two CTAs per SM (128-256 threads x 2-5 per SM measured: 93-102 us)
 template <int S, int NP, int MODE>
-__global__ void __launch_bounds__(MMX_L4_BLOCK, MMX_L4_MINB) k_local4(LocalArgs a) {
+__global__ void __launch_bounds__(MMX_L4_BLOCK, 2) k_local4(LocalArgs a) {
   // thread-private landing slots for the streamed inputs (B_demag, y0, k_j): cp.async puts them
   // in flight at the top of the kernel without holding registers; slot a of thread t is
   // lsm[a * 256 + t] (16 B per lane: conflict-free)
   extern __shared__ float4 lsm[];
   MmxCtrl* ctrl = a.ctrl;
-  pdl_wait();  // (multi-wave kernel: no early trigger, its own pending CTAs need the SM slots)
   if (!ctrl->active) return;
   const int sel = ctrl->sel;
   const size_t N = (size_t)a.nx * a.ny * a.nz;
   const unsigned gpr = a.nx >> 2;  // groups per row
-#if MMX_L4_EVICT
-  // (experiment, see MMX_L4_EVICT above) evict-first policy for data that is read once per call
-  unsigned long long pol_first;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_first));
-#endif
   auto stage3 = [&](int slot, const float* p, size_t idx) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
       const unsigned sa = (unsigned)__cvta_generic_to_shared(&lsm[(slot + c) * MMX_L4_BLOCK + threadIdx.x]);
-#if MMX_L4_EVICT
-      asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(p + (size_t)c * N + idx), "l"(pol_first) : "memory");
-#else
       asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(p + (size_t)c * N + idx) : "memory");
-#endif
     }
   };
   auto stq_stream = [&](float* p, size_t idx, const Q3& q) {
-#if MMX_L4_EVICT
-    const float4 vx = make_float4(q.c[0].x, q.c[1].x, q.c[2].x, q.c[3].x);
-    const float4 vy = make_float4(q.c[0].y, q.c[1].y, q.c[2].y, q.c[3].y);
-    const float4 vz = make_float4(q.c[0].z, q.c[1].z, q.c[2].z, q.c[3].z);
-    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p + idx), "f"(vx.x), "f"(vx.y), "f"(vx.z), "f"(vx.w), "l"(pol_first) : "memory");
-    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p + N + idx), "f"(vy.x), "f"(vy.y), "f"(vy.z), "f"(vy.w), "l"(pol_first) : "memory");
-    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p + 2 * N + idx), "f"(vz.x), "f"(vz.y), "f"(vz.z), "f"(vz.w), "l"(pol_first) : "memory");
-#else
     stq(p, N, idx, q);
-#endif
   };
   auto take3 = [&](int slot) -> Q3 {
     const float4 x = lsm[(slot + 0) * MMX_L4_BLOCK + threadIdx.x];
@@ -575,7 +545,6 @@ __global__ void __launch_bounds__(MMX_L4_BLOCK, MMX_L4_MINB) k_local4(LocalArgs 
 __global__ void __launch_bounds__(256) k_combine1(const float* y0a, const float* y0b, const float* k1a,
                                                   const float* k1b, float* yna, float* ynb, int row, int S,
                                                   int nvec, size_t N, MmxCtrl* ctrl) {
-  pdl_wait();
   if (!ctrl->active) return;
   const int sel = ctrl->sel;
   const float* y0 = sel ? y0b : y0a;
@@ -600,7 +569,6 @@ __global__ void __launch_bounds__(256) k_combine1(const float* y0a, const float*
 // mode 2: re-arm (active = 1) after a stepping call
 // mode 3: first step size from max torque: dt = 0.01 / max|tau| (only when dt <= 0)
 __global__ void k_controller(MmxCtrl* c, MmxTableau tab, int mode) {
-  pdl_wait();
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   if (mode == 2) { c->active = 1; return; }
   if (mode == 3) {

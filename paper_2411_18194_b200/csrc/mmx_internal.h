@@ -208,33 +208,9 @@ struct ProfScope {
   }
 };
 
-// ---- programmatic dependent launch (PDL) ---------------------------------------------------------
-// The kernels of a step run back to back on one stream.  Launched with the programmatic stream
-// serialization attribute, the CTAs of kernel B may start while the last CTAs of kernel A drain:
-// B does its independent preamble (twiddle tables, index arithmetic), then pdl_wait() blocks until A
-// has completed and its writes are visible.  Persistent kernels (all CTAs resident from the start)
-// call pdl_trigger() at the top, so B's CTAs take over SM by SM as A's CTAs exit; multi-wave kernels
-// do not trigger early (their own pending CTAs need the slots).  In a captured graph the attribute
-// becomes a programmatic dependency edge.
-// Measured on c4 (DP45 step, graph replay): plain launches 2.705 ms, PDL without early trigger
-// 2.706 ms, PDL with the early trigger in the persistent kernels 2.93 ms (the waiting CTAs of the next
-// kernel cost more than the hidden tails).  Off by default; -DMMX_PDL=1 / 2 to experiment.
-#ifndef MMX_PDL
-#define MMX_PDL 0
-#endif
 #ifdef __CUDACC__
-__device__ __forceinline__ void pdl_wait() {
-#if MMX_PDL
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-#endif
-}
-__device__ __forceinline__ void pdl_trigger() {
-#if MMX_PDL == 1
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-#endif
-}
-// grid of a persistent kernel: every CTA must be resident from the start (also a precondition of the
-// early pdl_trigger): CTAs per SM from the occupancy calculator, at most `want` per SM
+// grid of a persistent kernel: every CTA resident from the start; CTAs per SM from the occupancy
+// calculator, at most `want` per SM
 template <typename K>
 inline int mmx_persistent_grid(K kernel, int block, size_t smem, int sm_count, int want) {
   int per_sm = 0;
@@ -249,18 +225,8 @@ inline int mmx_persistent_grid(K kernel, int block, size_t smem, int sm_count, i
 template <typename... KArgs, typename... Args>
 inline cudaError_t mmx_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
                               Args... args) {
-#if MMX_PDL
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
-#else
   kernel<<<grid, block, smem, st>>>(KArgs(args)...);
   return cudaGetLastError();
-#endif
 }
 #endif
 
