@@ -633,7 +633,7 @@ int mmx_world_destroy(mmx_world* w) {
   for (int i = 0; i <= MMX_MAX_STAGES; ++i) cudaFree(w->K[i]);
   cudaFree(w->bdemag); cudaFree(w->strain); cudaFree(w->strain_f); cudaFree(w->scratch);
   for (int a = 0; a < 3; ++a) cudaFree(w->dm.tw[a]);
-  cudaFree(w->dm.spec1); cudaFree(w->dm.spec2); cudaFree(w->dm.khat);
+  cudaFree(w->dm.spec1); cudaFree(w->dm.spec2); cudaFree(w->dm.khat); cudaFree(w->dm.kimg);
   if (w->step_graph) cudaGraphExecDestroy(w->step_graph);
   if (w->own_stream) cudaStreamDestroy(w->stream);
   cudaGetLastError();
@@ -838,11 +838,20 @@ int mmx_demag_kernel_init(mmx_world* w, double analytic_cutoff_cells) {
   const double scale = -MU0 / ((double)d.px * d.py * d.pz);
   if (int rc = mmx_kernel_spectrum(w->grid, w->pbc, P, d.xp, oct, n, scale, khat)) return rc;
   cudaStreamSynchronize(w->stream);
-  if (!d.khat) {
-    if (int rc = dev_alloc(w, &d.khat, khat.size())) return rc;
+  // 3-D worlds with 128-point z lines on grids large enough for the pipelined y pass keep the padded
+  // spectrum tile-major and the kernel spectrum as per-tile images (demag_tile.cu)
+  d.tiled = mmx_tile_ok(d) && mmx_mid_col_ok(d.py, d.ny) && mmx_mid_pipe_ok(w, d.py, 3 * d.nz);
+  std::vector<float> kimg;
+  if (d.tiled) mmx_tile_kimg_build(d, khat, kimg);
+  if (!d.spec1) {
+    if (d.tiled) {
+      if (int rc = dev_alloc(w, &d.kimg, kimg.size())) return rc;
+    } else {
+      if (int rc = dev_alloc(w, &d.khat, khat.size())) return rc;
+    }
     if (int rc = dev_alloc(w, &d.spec1, (size_t)3 * d.nz * d.ny * d.xp)) return rc;
     if (d.nz > 1 && d.py > 1)
-      if (int rc = dev_alloc(w, &d.spec2, (size_t)3 * d.nz * d.py * d.xp)) return rc;
+      if (int rc = dev_alloc(w, &d.spec2, d.tiled ? mmx_tile_spec_elems(d.py, d.xc, d.nz) : (size_t)3 * d.nz * d.py * d.xp)) return rc;
     for (int a = 0; a < 3; ++a) {
       std::vector<float2> tw(P[a]);
       for (int q = 0; q < P[a]; ++q) {
@@ -853,7 +862,8 @@ int mmx_demag_kernel_init(mmx_world* w, double analytic_cutoff_cells) {
       MMX_CUDA(cudaMemcpy(d.tw[a], tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
     }
   }
-  MMX_CUDA(cudaMemcpy(d.khat, khat.data(), khat.size() * sizeof(float), cudaMemcpyHostToDevice));
+  if (d.tiled) MMX_CUDA(cudaMemcpy(d.kimg, kimg.data(), kimg.size() * sizeof(float), cudaMemcpyHostToDevice));
+  else MMX_CUDA(cudaMemcpy(d.khat, khat.data(), khat.size() * sizeof(float), cudaMemcpyHostToDevice));
   d.ready = true;
   w->k1_valid = false;
   w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale

@@ -375,7 +375,9 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ProfScope ps(w, PK_INNER);                                                             \
     k_inner<PP><<<g, block_for(PP), sm, st>>>(ia);                                        \
   }
-    if (mmx_inner_col_ok(d, Pin, ia.n_valid)) {
+    if (d.tiled) {
+      if (int rc = mmx_inner_tile_launch(w)) return rc;
+    } else if (mmx_inner_col_ok(d, Pin, ia.n_valid)) {
       InnerColLaunch L;
       L.spec = ia.spec; L.tw = ia.tw; L.n_valid = ia.n_valid; L.p_outer = ia.p_outer; L.n_outer = nouter;
       L.line_stride = ia.line_stride; L.comp_stride = ia.comp_stride; L.outer_stride = ia.outer_stride;

@@ -254,7 +254,13 @@ struct MidColArgs {
   int gated, n_in, n_out, xc, xp, nslab;
   int ntile_main, xc_main, nyq;
   size_t in_outer, out_outer;  // elements between consecutive (component, z) slabs
+  // tile-major layout of the padded side (demag_tile.cu), 0 = plain [slab][ky][xp]:
+  int t_nz;                    // z rows per component (slab = c nz + z)
+  unsigned t_tile, t_ks, t_nyq;  // complex elements per tile (3 nz 16), per ky (ntx tiles), offset of the Nyquist tiles
 };
+
+// position of column l (0..15) of a tile row with z index z: 16-byte chunks XOR-swizzled with (z & 7)
+__device__ __forceinline__ unsigned tile_pos16(unsigned l, unsigned z) { return ((((l >> 1) ^ (z & 7u)) << 1) | (l & 1u)); }
 
 // P = 2 R^2.  CTA = TILE columns x R threads per line x 2 halves; thread (kxl, j, h) transforms
 // half h (even / odd wave numbers) of the line of column kxl.
@@ -387,8 +393,15 @@ __global__ void __launch_bounds__(16 * R, 2) k_mid_pipe(MidColArgs a) {
       // from the uniform base (the launcher checks that they fit)
       constexpr int RPI = NT / (TL / 2);
       const unsigned ch = threadIdx.x % (TL / 2), r0 = threadIdx.x / (TL / 2);
-      const unsigned xp = (unsigned)a.xp;
-      const unsigned so = (unsigned)slab * (unsigned)a.in_outer + (unsigned)kx0 + r0 * xp + 2 * ch;
+      unsigned xp = (unsigned)a.xp;
+      unsigned so = (unsigned)slab * (unsigned)a.in_outer + (unsigned)kx0 + r0 * xp + 2 * ch;
+      if (DIR > 0 && a.t_nz) {
+        // rows are ky, the 64-byte half row of this tile holds its four chunks in swizzled order
+        const unsigned z = (unsigned)slab % (unsigned)a.t_nz;
+        const unsigned phys = ((((unsigned)kx0 >> 3) & 1u) * 4 + ch) ^ (z & 7u);
+        xp = a.t_ks;
+        so = ((unsigned)kx0 >> 4) * a.t_tile + (unsigned)slab * 16u + 2 * phys + r0 * xp;
+      }
 #pragma unroll
       for (int i = 0; i < ROWS / RPI; ++i) {
         const int row = r0 + RPI * i;
@@ -400,7 +413,11 @@ __global__ void __launch_bounds__(16 * R, 2) k_mid_pipe(MidColArgs a) {
         const int row = q / TL, l = q % TL;
         const bool v = row < a.n_in && slab0 + l < a.nslab;
         const int slab = v ? slab0 + l : 0;
-        cpa_zfill<8>(dst + row * TL + l, a.in + (size_t)slab * a.in_outer + (size_t)row * a.xp + (a.xc - 1), v);
+        const float2* src = a.in + (size_t)slab * a.in_outer + (size_t)row * a.xp + (a.xc - 1);
+        if (DIR > 0 && a.t_nz)
+          src = a.in + (a.t_nyq + ((unsigned)row >> 4) * a.t_tile + (unsigned)slab * 16u +
+                        tile_pos16((unsigned)row & 15u, (unsigned)slab % (unsigned)a.t_nz));
+        cpa_zfill<8>(dst + row * TL + l, src, v);
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
@@ -452,9 +469,19 @@ __global__ void __launch_bounds__(16 * R, 2) k_mid_pipe(MidColArgs a) {
     const unsigned oo = (unsigned)slab * (unsigned)a.out_outer + (unsigned)kx;
     if (DIR < 0) {
       if (ok) {
-        const unsigned o0 = oo + (unsigned)(2 * j + h) * xpu;
+        unsigned o0 = oo + (unsigned)(2 * j + h) * xpu, ostr = (unsigned)(2 * R) * xpu;
+        if (a.t_nz) {
+          const unsigned z = (unsigned)slab % (unsigned)a.t_nz, kyl = (unsigned)(2 * j + h);
+          if (tile < ntm) {  // row ky = kyl + 2 R b of tile column kx
+            o0 = ((unsigned)kx >> 4) * a.t_tile + (unsigned)slab * 16u + tile_pos16((unsigned)kx & 15u, z) + kyl * a.t_ks;
+            ostr = (unsigned)(2 * R) * a.t_ks;
+          } else {           // Nyquist column: tiles of 16 consecutive ky
+            o0 = a.t_nyq + (kyl >> 4) * a.t_tile + (unsigned)slab * 16u + tile_pos16(kyl & 15u, z);
+            ostr = (unsigned)(2 * R / 16) * a.t_tile;
+          }
+        }
 #pragma unroll
-        for (int b = 0; b < R; ++b) a.out[o0 + (unsigned)(2 * R * b) * xpu] = v[b];
+        for (int b = 0; b < R; ++b) a.out[o0 + (unsigned)b * ostr] = v[b];
       }
     } else {
       // x[n] = g0[n] + conj(w_P^n) g1[n]: lanes h = 0 finish rows b < R/2, lanes h = 1 the others
@@ -523,6 +550,13 @@ int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L) {
 
 bool mmx_mid_col_ok(int P, int n) { return (P == 512 || P == 128 || P == 32) && 2 * n <= P; }
 
+// the pipelined y pass (k_mid_pipe) serves 512-point lines on grids with enough tiles to fill the GPU
+bool mmx_mid_pipe_ok(const mmx_world* w, int P, int nslab) {
+  const DemagPlan& d = w->dm;
+  const long long ntiles = (long long)((d.xc + 15) / 16) * nslab;
+  return P == 512 && ntiles >= 8LL * w->sm_count && (size_t)nslab * d.py * d.xp < (1ull << 31);
+}
+
 template <int R, int TILE>
 static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
   a.nyq = ((a.xc - 1) % TILE == 0 && a.xc > 1 && a.nslab >= TILE) ? 1 : 0;
@@ -532,8 +566,7 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
   const size_t smem = sizeof(float2) * (dir < 0 ? 2 : 3) * R * R * TILE;
   ProfScope ps(w, dir < 0 ? PK_MID_FWD : PK_MID_INV);
   const int ntiles = a.ntile_main * a.nslab + (a.nyq ? (a.nslab + TILE - 1) / TILE : 0);
-  if (R == 16 && ntiles >= 8 * w->sm_count && (size_t)a.nslab * a.out_outer < (1ull << 31) &&
-      (size_t)a.nslab * a.in_outer < (1ull << 31)) {
+  if (R == 16 && mmx_mid_pipe_ok(w, 2 * R * R, a.nslab)) {
     MidColArgs b = a;
     constexpr int TL = 8;
     b.nyq = ((a.xc - 1) % TL == 0 && a.xc > 1 && a.nslab >= TL) ? 1 : 0;
@@ -554,6 +587,7 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
     return MMX_OK;
   }
   (void)ntiles;
+  if (a.t_nz) return mmx_fail(MMX_EINVAL, "mid column pass: the tile-major layout needs the pipelined kernel");
   if (dir < 0) {
     if (int rc = set_smem_col(k_mid_col<R, TILE, -1>, smem)) return rc;
     k_mid_col<R, TILE, -1><<<g, 2 * R * TILE, smem, w->stream>>>(a);
@@ -572,6 +606,13 @@ int mmx_mid_col_launch(mmx_world* w, int P, int dir, const float2* in, float2* o
   a.in = in; a.out = out; a.tw = tw; a.ctrl = w->d_ctrl; a.gated = 1;
   a.n_in = n_in; a.n_out = n_out; a.xc = d.xc; a.xp = d.xp; a.nslab = nslab;
   a.in_outer = in_outer; a.out_outer = out_outer;
+  a.t_nz = 0; a.t_tile = a.t_ks = a.t_nyq = 0;
+  if (d.tiled) {  // the padded side (spec2) is tile-major: demag_tile.cu
+    a.t_nz = d.nz;
+    a.t_tile = 3u * d.nz * 16u;
+    a.t_ks = (unsigned)((d.xc - 1) / 16) * a.t_tile;
+    a.t_nyq = (unsigned)d.py * a.t_ks;
+  }
   switch (P) {
     case 512: return mid_col_launch_t<16, 16>(w, a, dir);
     case 128: return mid_col_launch_t<8, 32>(w, a, dir);

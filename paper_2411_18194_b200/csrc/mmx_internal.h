@@ -125,6 +125,8 @@ struct DemagPlan {
   float2* spec1;       // [3][nz][ny][xp]
   float2* spec2;       // [3][nz][py][xp]  (3-D only)
   float* khat;         // [6][kz][ky][xp]
+  bool tiled;          // 3-D fast path: spec2 is tile-major and the kernel spectrum is stored as images (demag_tile.cu)
+  float* kimg;         // [(py/2+1) ntx + py/16][6][65][16] (tiled only; khat is then not kept on the device)
   bool ready;
 };
 
@@ -263,6 +265,14 @@ struct InnerColLaunch {
 bool mmx_inner_col_ok(const DemagPlan& d, int P, int n_valid);
 int mmx_inner_col_launch(mmx_world* w, const InnerColLaunch& L);
 bool mmx_mid_col_ok(int P, int n);
+bool mmx_mid_pipe_ok(const mmx_world* w, int P, int nslab);
+
+// demag_tile.cu: fused inner pass on the tile-major spectrum (3-D worlds with Pz = 128 on large grids)
+bool mmx_tile_ok(const DemagPlan& d);
+size_t mmx_tile_spec_elems(int py, int xc, int nz);
+size_t mmx_tile_kimg_floats(int py, int xc);
+void mmx_tile_kimg_build(const DemagPlan& d, const std::vector<float>& khat, std::vector<float>& out);
+int mmx_inner_tile_launch(mmx_world* w);
 int mmx_mid_col_launch(mmx_world* w, int P, int dir, const float2* in, float2* out, int n_in, int n_out,
                        size_t in_outer, size_t out_outer, int nslab, const float2* tw);
 
