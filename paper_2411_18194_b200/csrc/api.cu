@@ -214,6 +214,7 @@ int alloc_state(mmx_world* w) {
   w->sel_host = 0;
   w->k1_valid = false;
   w->cfg_epoch++;
+  w->n_tmaps = 0;  // the buffers moved
   // ctrl->sel must follow
   int zero = 0;
   MMX_CUDA(cudaMemcpyAsync(&w->d_ctrl->sel, &zero, sizeof(int), cudaMemcpyHostToDevice, w->stream));
@@ -575,6 +576,7 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
   w->has_dmiq = false;
   for (int s = 0; s < 2; ++s)
     for (int k = 0; k < 9; ++k) w->dmiq[s][k] = 0.0;
+  w->n_tmaps = 0;
   w->step_graph = nullptr; w->graph_method = -1; w->graph_epoch = -1; w->cfg_epoch = 0; w->graph_launches = 0;
   w->use_graphs = getenv("MMX_NO_GRAPH") == nullptr;
   {

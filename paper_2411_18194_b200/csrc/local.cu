@@ -18,6 +18,9 @@
 // the region-pair scale factor across grain boundaries.
 // The epilogue forms the next stage state  normalise(y0 + sum_j (dt a_ij) k_j)  (Table 2,
 // P:L122-131) and, on the last stage, the embedded error  max_c |sum_j (dt e_j) k_j|_2.
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include <cstdio>
 
 #include "mmx_internal.h"
@@ -541,6 +544,259 @@ __global__ void __launch_bounds__(MMX_L4_BLOCK, 2) k_local4(LocalArgs a) {
   if (a.do_tq) block_max_to(tqv, &ctrl->tq_bits);
 }
 
+// ---- TMA halo-tile path: one sublattice, uniform material, open boundaries (the c4 / c1 shape) --------
+// A CTA owns a tile of 64 x 4 x 2 cells.  The tile of m with its one-cell halo arrives in shared memory by
+// ONE tensor-map TMA copy (cp.async.bulk.tensor.4d, box 72 x 6 x 4 x 3 floats starting at x0 - 4 so that a
+// thread's four cells are a 16-byte aligned LDS.128; cells outside the grid are zero-filled by the copy
+// unit and masked by the validity flags below, which is the "open" boundary of S9): the centre and all
+// six neighbours are shared-memory reads, no register is held for a load in flight and there is no
+// per-thread address arithmetic for the stencil.  The streamed inputs (B_demag, y0, k_j) keep their
+// thread-private cp.async landing slots; outputs are float4 stores.  Same arithmetic, term by term, as
+// k_local4 / k_local.  Three to five CTAs of 128 threads per SM.
+constexpr int LT_TX = 64, LT_TY = 4, LT_TZ = 2, LT_BX = 72, LT_BY = LT_TY + 2, LT_BZ = LT_TZ + 2, LT_NT = 128;
+constexpr int LT_HALO_BYTES = 3 * LT_BZ * LT_BY * LT_BX * 4;  // 20736
+
+__device__ __forceinline__ unsigned lt_s32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <int NP, int MODE>
+__global__ void __launch_bounds__(LT_NT, 3) k_local_t(LocalArgs a, const __grid_constant__ CUtensorMap tm0,
+                                                      const __grid_constant__ CUtensorMap tm1) {
+  extern __shared__ __align__(128) unsigned char smraw[];
+  float* halo = reinterpret_cast<float*>(smraw);                             // [3][BZ][BY][BX]
+  float4* lsm = reinterpret_cast<float4*>(smraw + LT_HALO_BYTES);             // landing slots [slot][NT]
+  __shared__ __align__(8) unsigned long long bar;
+  MmxCtrl* ctrl = a.ctrl;
+  if (!ctrl->active) return;
+  const int sel = ctrl->sel;
+  const size_t N = (size_t)a.nx * a.ny * a.nz;
+  const int x0 = blockIdx.x * LT_TX, y0 = blockIdx.y * LT_TY, z0 = blockIdx.z * LT_TZ;
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(lt_s32(&bar)) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const CUtensorMap* tm = sel ? &tm1 : &tm0;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(lt_s32(&bar)), "r"(LT_HALO_BYTES) : "memory");
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(lt_s32(halo)), "l"(tm), "r"(x0 - 4), "r"(y0 - 1), "r"(z0 - 1), "r"(0), "r"(lt_s32(&bar)) : "memory");
+  }
+  const int tx = threadIdx.x & 15, ty = (threadIdx.x >> 4) & 3, tz = threadIdx.x >> 6;
+  const int ix = x0 + 4 * tx, iy = y0 + ty, iz = z0 + tz;
+  const bool inside = ix < a.nx && iy < a.ny && iz < a.nz;
+  const size_t i = ((size_t)iz * a.ny + iy) * a.nx + ix;
+  auto stage3 = [&](int slot, const float* p, size_t idx) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const unsigned sa = lt_s32(&lsm[(slot + c) * LT_NT + threadIdx.x]);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(p + (size_t)c * N + idx) : "memory");
+    }
+  };
+  auto take3 = [&](int slot) -> Q3 {
+    const float4 x = lsm[(slot + 0) * LT_NT + threadIdx.x];
+    const float4 y = lsm[(slot + 1) * LT_NT + threadIdx.x];
+    const float4 z = lsm[(slot + 2) * LT_NT + threadIdx.x];
+    Q3 q;
+    q.c[0] = v3(x.x, y.x, z.x); q.c[1] = v3(x.y, y.y, z.y); q.c[2] = v3(x.z, y.z, z.z); q.c[3] = v3(x.w, y.w, z.w);
+    return q;
+  };
+  constexpr bool comb = (MODE & 1) != 0, doerr = (MODE & 2) != 0;
+  const bool epi = !a.heff_out && !a.tau_out;
+  const float* ca = ctrl->ca[a.combine_row];
+  const float* ce = ctrl->ce;
+  const bool use_bd = (a.terms & MMX_T_DEMAG) && a.bdemag;
+  if (inside) {
+    // streamed inputs: slot 0 B_demag, slot 3 y0, slot 6 + 3 j k_j
+    if (use_bd) stage3(0, a.bdemag, i);
+    if (MODE != 0 && epi) {
+      if (comb) stage3(3, a.y0[sel], i);
+#pragma unroll
+      for (int j = 0; j < NP; ++j) {
+        const float cj = comb ? ca[j] : 0.f;
+        const float ej = doerr ? ce[j] : 0.f;
+        if (cj != 0.f || ej != 0.f) stage3(6 + 3 * j, a.kprev[sel][j], i);
+      }
+    }
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  {  // the halo tile has landed
+    unsigned ok = 0;
+    for (int spin = 0; !ok; ++spin) {
+      asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}\n"
+                   : "=r"(ok) : "r"(lt_s32(&bar)) : "memory");
+      if (!ok && spin > (1 << 22)) __trap();
+    }
+  }
+  float errv = 0.f, tqv = 0.f;
+  bool bad = false;
+  if (inside) {
+    auto hq = [&](int dz, int dy) -> Q3 {  // the thread's four cells of row (ty + dy, tz + dz)
+      const float* p = halo + ((tz + 1 + dz) * LT_BY + (ty + 1 + dy)) * LT_BX + 4 + 4 * tx;
+      const float4 x = *reinterpret_cast<const float4*>(p);
+      const float4 y = *reinterpret_cast<const float4*>(p + LT_BZ * LT_BY * LT_BX);
+      const float4 z = *reinterpret_cast<const float4*>(p + 2 * LT_BZ * LT_BY * LT_BX);
+      Q3 q;
+      q.c[0] = v3(x.x, y.x, z.x); q.c[1] = v3(x.y, y.y, z.y); q.c[2] = v3(x.z, y.z, z.z); q.c[3] = v3(x.w, y.w, z.w);
+      return q;
+    };
+    auto h1 = [&](int xo) -> V3 {  // one cell of the thread's own row at x offset xo from its first cell
+      const float* p = halo + ((tz + 1) * LT_BY + (ty + 1)) * LT_BX + 4 + 4 * tx + xo;
+      return v3(p[0], p[LT_BZ * LT_BY * LT_BX], p[2 * LT_BZ * LT_BY * LT_BX]);
+    };
+    const bool val[6] = {ix + 4 < a.nx, ix > 0, iy + 1 < a.ny, iy > 0, iz + 1 < a.nz, iz > 0};
+    const Q3 mc = hq(0, 0);
+    const float* P = a.mat;
+    const float iMs = P[MP_INVMS];
+    Q3 B, dm;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) { B.c[e] = v3(0.f, 0.f, 0.f); dm.c[e] = v3(0.f, 0.f, 0.f); }
+    const float Ac = P[MP_A], Dc = P[MP_D], zlb = P[MP_ZLB];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+      const int axis = q >> 1;
+      const float d = (q & 1) ? -1.f : 1.f;
+      Q3 mn;
+      bool v[4] = {val[q], val[q], val[q], val[q]};
+      if (q == 0) {
+        mn.c[0] = mc.c[1]; mn.c[1] = mc.c[2]; mn.c[2] = mc.c[3]; mn.c[3] = h1(4);
+        v[0] = v[1] = v[2] = true;
+      } else if (q == 1) {
+        mn.c[3] = mc.c[2]; mn.c[2] = mc.c[1]; mn.c[1] = mc.c[0]; mn.c[0] = h1(-1);
+        v[1] = v[2] = v[3] = true;
+      } else {
+        mn = hq(axis == 2 ? (q == 4 ? 1 : -1) : 0, axis == 1 ? (q == 2 ? 1 : -1) : 0);
+      }
+      const float wex = 2.f * harm(Ac, Ac) * iMs * a.inv_h2[axis];
+      const float wd = harm(Dc, Dc) * iMs * a.inv_h[axis] * d;
+      const float wu = zlb * a.J[axis] * 0.5f * a.inv_h[axis] * d;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        if (v[e]) {
+          if (a.terms & MMX_T_EXCH) B.c[e] = fma3(wex, mn.c[e] - mc.c[e], B.c[e]);
+          if (axis < 2 && (a.terms & MMX_T_DMI)) {
+            if (axis == 0) { B.c[e].x = fmaf(wd, mn.c[e].z, B.c[e].x); B.c[e].z = fmaf(-wd, mn.c[e].x, B.c[e].z); }
+            else { B.c[e].y = fmaf(wd, mn.c[e].z, B.c[e].y); B.c[e].z = fmaf(-wd, mn.c[e].y, B.c[e].z); }
+          }
+        }
+        if (a.has_J) dm.c[e] = fma3(wu, v[e] ? mn.c[e] : mc.c[e], dm.c[e]);
+      }
+    }
+    Q3 bd, tau;
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (use_bd) bd = take3(0);
+    float eps[6][4];
+    const bool use_mel = (a.terms & MMX_T_MEL) && a.strain;
+    if (use_mel) {
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        const float4 t = *reinterpret_cast<const float4*>(a.strain + (size_t)c * N + i);
+        eps[c][0] = t.x; eps[c][1] = t.y; eps[c][2] = t.z; eps[c][3] = t.w;
+      }
+    }
+    const float alpha = P[MP_ALPHA], llg = P[MP_LLG], xi = P[MP_XI];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const V3 m = mc.c[e];
+      V3 Bc = B.c[e];
+      if (a.terms & MMX_T_ANIS_U) {
+        const V3 u = v3(P[MP_UX], P[MP_UY], P[MP_UZ]);
+        Bc = fma3(P[MP_KU2] * dot(u, m), u, Bc);
+      }
+      if ((a.terms & MMX_T_ANIS_C) && P[MP_KC2] != 0.f) {
+        const V3 c1 = v3(P[MP_C1X], P[MP_C1Y], P[MP_C1Z]);
+        const V3 c2 = v3(P[MP_C2X], P[MP_C2Y], P[MP_C2Z]);
+        const V3 c3 = v3(P[MP_C3X], P[MP_C3Y], P[MP_C3Z]);
+        const float a1 = dot(c1, m), a2 = dot(c2, m), a3 = dot(c3, m);
+        const float k = -P[MP_KC2];
+        Bc = fma3(k * a1 * (a2 * a2 + a3 * a3), c1, Bc);
+        Bc = fma3(k * a2 * (a3 * a3 + a1 * a1), c2, Bc);
+        Bc = fma3(k * a3 * (a1 * a1 + a2 * a2), c3, Bc);
+      }
+      if (a.terms & MMX_T_ZEEMAN) Bc = Bc + v3(a.bext[0], a.bext[1], a.bext[2]);
+      if (use_bd) Bc = Bc + bd.c[e];
+      if (use_mel) {
+        const float p1 = -P[MP_MEL1], p2 = -P[MP_MEL2];
+        Bc.x += p1 * eps[0][e] * m.x + p2 * (eps[3][e] * m.y + eps[4][e] * m.z);
+        Bc.y += p1 * eps[1][e] * m.y + p2 * (eps[3][e] * m.x + eps[5][e] * m.z);
+        Bc.z += p1 * eps[2][e] * m.z + p2 * (eps[4][e] * m.x + eps[5][e] * m.y);
+      }
+      B.c[e] = Bc;
+      const V3 mxB = cross(m, Bc);
+      const V3 mxmxB = cross(m, mxB);
+      V3 t = (-llg) * fma3(alpha, mxmxB, mxB);
+      if (a.has_J) {
+        const V3 mxa = cross(m, dm.c[e]);
+        const V3 mxmxa = cross(m, mxa);
+        const float inv = -1.f / (1.f + alpha * alpha);
+        t = fma3(inv * (1.f + xi * alpha), mxmxa, t);
+        t = fma3(inv * (xi - alpha), mxa, t);
+      }
+      tau.c[e] = t;
+    }
+    if (a.heff_out) stq(a.heff_out, N, i, B);
+    else if (a.tau_out) stq(a.tau_out, N, i, tau);
+    else {
+      stq(a.kout[sel], N, i, tau);
+      if (a.do_tq) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float t2 = dot(tau.c[e], tau.c[e]);
+          tqv = fmaxf(tqv, sqrtf(t2));
+          bad |= !(t2 == t2);
+        }
+      }
+      Q3 ys, er;
+      if (MODE != 0) {
+        if (comb) ys = take3(3);
+        if (doerr) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) er.c[e] = v3(0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int j = 0; j < NP; ++j) {
+          const float cj = comb ? ca[j] : 0.f;
+          const float ej = doerr ? ce[j] : 0.f;
+          if (cj != 0.f || ej != 0.f) {
+            const Q3 kj = take3(6 + 3 * j);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              if (comb) ys.c[e] = fma3(cj, kj.c[e], ys.c[e]);
+              if (doerr) er.c[e] = fma3(ej, kj.c[e], er.c[e]);
+            }
+          }
+        }
+      }
+      if (comb) {
+        const float cs = ca[a.stage];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          V3 yy = fma3(cs, tau.c[e], ys.c[e]);
+          const float n2 = dot(yy, yy);
+          if (n2 > 0.f) yy = (1.f / sqrtf(n2)) * yy;
+          ys.c[e] = yy;
+        }
+        stq(a.ynext[sel], N, i, ys);
+      }
+      if (doerr) {
+        const float es = ce[a.stage];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const V3 ee = fma3(es, tau.c[e], er.c[e]);
+          const float e2 = dot(ee, ee);
+          errv = fmaxf(errv, sqrtf(e2));
+          bad |= !(e2 == e2);
+        }
+      }
+    }
+  } else {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+  }
+  if (bad) errv = tqv = __int_as_float(0x7fc00000);
+  if (a.do_err) block_max_to(errv, &ctrl->err_bits);
+  if (a.do_tq) block_max_to(tqv, &ctrl->tq_bits);
+}
+
 // y_next = project(y0 + ca[row][0] * k1) for all vectors (m normalised, u and v not)
 __global__ void __launch_bounds__(256) k_combine1(const float* y0a, const float* y0b, const float* k1a,
                                                   const float* k1b, float* yna, float* ynb, int row, int S,
@@ -663,6 +919,34 @@ __global__ void __launch_bounds__(256) k_dot_energy(const float* m, const float*
 
 }  // namespace
 
+// tensor map of a state buffer [3 nvec][nz][ny][nx] floats with the halo box of k_local_t
+static int tmap_for(mmx_world* w, const float* base, const CUtensorMap** out) {
+  for (int k = 0; k < w->n_tmaps; ++k)
+    if (w->tmaps[k].base == base) { *out = reinterpret_cast<const CUtensorMap*>(w->tmaps[k].bytes); return MMX_OK; }
+  if (w->n_tmaps >= 4) w->n_tmaps = 0;
+  static PFN_cuTensorMapEncodeTiled encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn)
+      return mmx_fail(MMX_ECUDA, "cuTensorMapEncodeTiled is not available");
+    encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(fn);
+  }
+  MmxTmap& t = w->tmaps[w->n_tmaps];
+  const cuuint64_t dims[4] = {(cuuint64_t)w->grid[0], (cuuint64_t)w->grid[1], (cuuint64_t)w->grid[2], (cuuint64_t)(3 * w->nvec)};
+  const cuuint64_t strides[3] = {(cuuint64_t)w->grid[0] * 4, (cuuint64_t)w->grid[0] * w->grid[1] * 4, (cuuint64_t)w->N * 4};
+  const cuuint32_t box[4] = {LT_BX, LT_BY, LT_BZ, 3};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const CUresult r = encode(reinterpret_cast<CUtensorMap*>(t.bytes), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(base), dims,
+                            strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return mmx_fail(MMX_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  t.base = base;
+  w->n_tmaps++;
+  *out = reinterpret_cast<const CUtensorMap*>(t.bytes);
+  return MMX_OK;
+}
+
 int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   const size_t N = w->N;
   const unsigned blocks = (unsigned)((N + 255) / 256);
@@ -670,7 +954,32 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   ProfScope ps(w, PK_LOCAL);
   bool uniform = !reg && (w->grid[0] % 4) == 0 && !a.has_dmiq;  // (the general DMI tensor lives in k_local only)
   for (int s = 0; s < w->S && uniform; ++s) uniform = w->mats[(size_t)s * w->nreg].Ms > 0;
-  if (uniform) {
+  const bool open_all = !a.per[0] && !a.per[1] && !a.per[2];
+  if (uniform && w->S == 1 && open_all) {
+    // TMA halo tiles (k_local_t)
+    const CUtensorMap *m0, *m1;
+    if (int rc = tmap_for(w, a.yin[0], &m0)) return rc;
+    if (int rc = tmap_for(w, a.yin[1], &m1)) return rc;
+    const CUtensorMap t0 = *m0, t1 = *m1;  // (copies: a second lookup may recycle the cache slot)
+    const dim3 grid((w->grid[0] + LT_TX - 1) / LT_TX, (w->grid[1] + LT_TY - 1) / LT_TY, (w->grid[2] + LT_TZ - 1) / LT_TZ);
+    const int mode = (a.ynext[0] ? 1 : 0) | (a.do_err ? 2 : 0);
+#define MMX_LT_GO(NP_, M_)                                                                                         \
+  {                                                                                                                \
+    const size_t sm_ = LT_HALO_BYTES + sizeof(float4) * LT_NT * (6 + 3 * (NP_));                                   \
+    if (sm_ > 32 * 1024)                                                                                           \
+      MMX_CUDA(cudaFuncSetAttribute(k_local_t<NP_, M_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_));   \
+    k_local_t<NP_, M_><<<grid, LT_NT, sm_, w->stream>>>(a, t0, t1);                                                \
+  }
+#define MMX_LT(NP_)                                \
+  case NP_:                                        \
+    if (mode == 0) MMX_LT_GO(0, 0)                 \
+    else if (mode == 1) MMX_LT_GO(NP_, 1)          \
+    else if (mode == 2) MMX_LT_GO(NP_, 2)          \
+    else MMX_LT_GO(NP_, 3)                         \
+    break;
+    switch (a.n_prev) { MMX_LT(0) MMX_LT(1) MMX_LT(2) MMX_LT(3) MMX_LT(4) MMX_LT(5) MMX_LT(6) MMX_LT(7)
+      default: return mmx_fail(MMX_EINVAL, "n_prev %d out of range", a.n_prev); }
+  } else if (uniform) {
     const unsigned b4 = (unsigned)((N / 4 + MMX_L4_BLOCK - 1) / MMX_L4_BLOCK);
     const int mode = (a.ynext[0] ? 1 : 0) | (a.do_err ? 2 : 0);
 #define MMX_L4_GO(S_, NP_, M_)                                                             \

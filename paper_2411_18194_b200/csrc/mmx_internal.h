@@ -139,6 +139,12 @@ struct ProfRec {
   cudaEvent_t e0, e1;
 };
 
+// a tensor map (CUtensorMap, 128 bytes) of one state buffer, for the TMA halo tiles of local.cu
+struct MmxTmap {
+  alignas(64) unsigned char bytes[128];
+  const float* base;
+};
+
 struct mmx_world {
   int grid[3];
   double cell[3];
@@ -187,6 +193,8 @@ struct mmx_world {
   long long graph_epoch, cfg_epoch;   // the graph is valid while graph_epoch == cfg_epoch
   long long graph_launches;           // kernels per replay
   bool use_graphs;
+  MmxTmap tmaps[4];    // state buffers seen by the TMA local kernel (Y[0..1], YS[0..1]); reset by alloc_state
+  int n_tmaps;
 };
 
 // RAII: brackets one kernel launch with CUDA events on the world's stream when profiling is on
