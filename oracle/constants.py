@@ -5,6 +5,7 @@ MU0 = 4e-7 * math.pi          # T m / A (S2)
 GAMMA = 1.7595e11             # rad / (T s) (S1; per-material parameter, this is the default)
 MU_B = 9.2740100783e-24       # J / T
 Q_E = 1.602176634e-19         # C
+HBAR = 1.054571817e-34        # J s
 
 # effective-field term bits (same numbering as include/mmx.h)
 T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0, T_DMI_INTER, T_MEL, T_DMI_HOMO = (

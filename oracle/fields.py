@@ -13,7 +13,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from .constants import MU_B, Q_E
+from .constants import HBAR, MU_B, Q_E
 
 
 # ----------------------------------------------------------------------
@@ -218,3 +218,22 @@ def zhang_li_torque(m, Ms, alpha, pol, xi, J, cell, pbc):
     mxmxa = cross(m, mxa)
     return (-1.0 / (1.0 + alpha * alpha))[None] * ((1.0 + xi * alpha)[None] * mxmxa
                                                    + (xi - alpha)[None] * mxa)
+
+
+def slonczewski_torque(m, Ms, alpha, gamma, pol, jz, mp, lam, eps_prime, thickness):
+    """Slonczewski spin-transfer torque ("as formulated by ... Slonczewski [29], implemented in
+    the same way as in mumax3"; the paper prints no formula -- reading S37).  In Gilbert form a current
+    density jz through a free layer of thickness d, polarised along the fixed-layer direction m_p, adds
+        T = gamma beta [ eps m x (m_p x m) - eps' m x m_p ],     beta = hbar jz / (e Ms d)   [T]
+        eps = P Lambda^2 / ((Lambda^2 + 1) + (Lambda^2 - 1) (m . m_p))
+    to  dm/dt = -gamma m x B + alpha m x dm/dt + T.  Solving for dm/dt (as for Eq.2) gives the explicit torque
+        tau_SL = gamma beta / (1 + alpha^2) [ (eps + alpha eps') m x (m_p x m) - (eps' - alpha eps) m x m_p ].
+    m_p [3] unit vector; returns 1/s."""
+    mpv = np.asarray(mp, float).reshape(3, 1, 1, 1) * np.ones_like(m)
+    beta = HBAR * jz / (Q_E * thickness) * _inv(Ms)
+    l2 = lam * lam
+    eps = pol * l2 / ((l2 + 1.0) + (l2 - 1.0) * (m * mpv).sum(axis=0))
+    pxm = cross(mpv, m)
+    mxpxm = cross(m, pxm)
+    pref = gamma * beta / (1.0 + alpha * alpha)
+    return (pref * (eps + alpha * eps_prime))[None] * mxpxm + (pref * (eps_prime - alpha * eps))[None] * pxm

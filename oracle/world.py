@@ -131,6 +131,11 @@ class World:
         if any(j != 0.0 for j in self.J):
             tau = tau + fl.zhang_li_torque(m[s], p["Ms"], p["alpha"], p["pol"], p["xi"], self.J,
                                            self.cell, self.pbc)
+        sl = self.cpl.get("slonczewski")
+        if sl and sl["jz"] != 0.0:   # reading S37
+            d = sl.get("thickness") or self.grid[2] * self.cell[2]
+            tau = tau + fl.slonczewski_torque(m[s], p["Ms"], p["alpha"], p["gamma"], p["pol"], sl["jz"], sl["mp"],
+                                              sl.get("lambda", 1.0), sl.get("eps_prime", 0.0), d)
         return tau * (p["Ms"] > 0)[None]
 
     # ------------------------------------------------------------------ elastic

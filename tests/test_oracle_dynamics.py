@@ -268,3 +268,67 @@ def test_P13_zhang_li():
     w.step_rk4(5e-14, int(round(T / 5e-14)))
     q1 = 0.5 * (nx * h - w.m[0][2].sum() * h)
     assert abs((q1 - q0) / T + u) < 0.02 * u
+
+
+def test_P23_slonczewski_macrospin_closed_form():
+    """P23 (pins reading S37: prefactor hbar/(e Ms d), eps(Lambda = 1) = P/2, the alpha mixing and the role of eps').
+    Macrospin in B z^ with the fixed layer along z^ and Lambda = 1: from the Gilbert form
+    dm/dt = -gamma m x B + alpha m x dm/dt + gamma beta [eps m x (z x m) - eps' m x z] one gets, exactly,
+        m_z(t) = tanh( gamma (alpha (B + beta eps') + beta eps) t / (1 + alpha^2) + atanh m_z(0) )
+        dphi/dt = gamma ((B + beta eps') - alpha beta eps) / (1 + alpha^2)
+    so the damping-like torque cancels the Gilbert damping at beta eps = -alpha (B + beta eps') (switching current)."""
+    from oracle.constants import HBAR, Q_E
+    Ms, alpha, P, d, B, epsp = 8.0e5, 0.02, 0.4, 2e-9, 0.2, 0.05
+    spec = wl.make("c1", (1, 1, 1))
+    spec.demag = False
+    spec.mat["alpha"][:] = alpha
+    spec.mat["pol"][:] = P
+    spec.mat["A"][:] = 0.0
+    spec.bext = (0.0, 0.0, B)
+    m0 = np.array([np.sin(0.6), 0.0, np.cos(0.6)])
+    for jz in (-3.0e11, +2.0e11, 0.0):
+        s2 = spec.copy()
+        s2.m = [m0.reshape(3, 1, 1, 1).astype(np.float32)]
+        s2.coupling["slonczewski"] = dict(jz=jz, mp=(0.0, 0.0, 1.0), **{"lambda": 1.0}, eps_prime=epsp, thickness=d)
+        o = World(s2)
+        beta = HBAR * jz / (Q_E * Ms * d)
+        eps = P / 2.0
+        rate = GAMMA * (alpha * (B + beta * epsp) + beta * eps) / (1 + alpha ** 2)
+        omega = GAMMA * ((B + beta * epsp) - alpha * beta * eps) / (1 + alpha ** 2)
+        dt, n = 2e-14, 2000
+        o.step_rk4(dt, n)
+        t = n * dt
+        mz = np.tanh(rate * t + np.arctanh(float(o.spec.m[0][2, 0, 0, 0])))
+        phi = np.arctan2(o.m[0][1, 0, 0, 0], o.m[0][0, 0, 0, 0])
+        assert abs(o.m[0][2, 0, 0, 0] - mz) < 1e-7, (jz, o.m[0][2, 0, 0, 0], mz)
+        assert abs(np.angle(np.exp(1j * (phi - omega * t)))) < 1e-6, (jz, phi, omega * t)
+    # the damping-like torque exactly compensates the Gilbert damping at the switching current
+    jc = -alpha * B * Q_E * Ms * d / (HBAR * (P / 2.0 + alpha * epsp))
+    s2 = spec.copy()
+    s2.m = [m0.reshape(3, 1, 1, 1).astype(np.float32)]
+    s2.coupling["slonczewski"] = dict(jz=jc, mp=(0.0, 0.0, 1.0), **{"lambda": 1.0}, eps_prime=epsp, thickness=d)
+    o = World(s2)
+    assert abs(o.torque(0)[2, 0, 0, 0]) < 1e-6 * GAMMA * B
+
+
+def test_slonczewski_angular_dependence():
+    """eps(m . m_p) of reading S37 at its three closed-form points: P/2 (parallel), P Lambda^2/2 (antiparallel),
+    P Lambda^2/(Lambda^2 + 1) (perpendicular) -- read off the torque on a spin perpendicular to m_p, and the
+    vanishing torque at m = +-m_p."""
+    from oracle import fields as fl
+    from oracle.constants import HBAR, Q_E
+    Ms, P, lam, d, jz = 5.0e5, 0.6, 1.7, 3e-9, 1e11
+    one = lambda v: np.asarray(v, float).reshape(3, 1, 1, 1)
+    arr = lambda x: np.full((1, 1, 1), float(x))
+    beta = HBAR * jz / (Q_E * Ms * d)
+    tau = fl.slonczewski_torque(one((1, 0, 0)), arr(Ms), arr(0.0), arr(GAMMA), arr(P), jz, (0, 0, 1), lam, 0.0, d)
+    # m = x^, m_p = z^, alpha = 0: tau = gamma beta eps (z - 0) = gamma beta eps z^, eps = P L^2/(L^2+1)
+    np.testing.assert_allclose(tau[:, 0, 0, 0], [0, 0, GAMMA * beta * P * lam ** 2 / (lam ** 2 + 1)], rtol=1e-12, atol=1e-3)
+    for sgn in (+1, -1):
+        tau = fl.slonczewski_torque(one((0, 0, sgn)), arr(Ms), arr(0.1), arr(GAMMA), arr(P), jz, (0, 0, 1), lam, 0.3, d)
+        assert np.abs(tau).max() == 0.0
+    th = 1e-6   # nearly (anti)parallel: |tau| / sin(theta) -> gamma beta eps(+-1)
+    for sgn, eps in ((+1, P / 2), (-1, P * lam ** 2 / 2)):
+        m = one((np.sin(th), 0, sgn * np.cos(th)))
+        tau = fl.slonczewski_torque(m, arr(Ms), arr(0.0), arr(GAMMA), arr(P), jz, (0, 0, 1), lam, 0.0, d)
+        np.testing.assert_allclose(np.sqrt((tau ** 2).sum()) / np.sin(th), GAMMA * abs(beta) * eps, rtol=1e-5)
