@@ -109,6 +109,14 @@ class World:
             if terms & T_DMI_INTER:
                 Di = np.full_like(p["Ms"], self.cpl["D_inter"])
                 out[T_DMI_INTER] = fl.dmi_interfacial(m[o], p["Ms"], Di, self.cell, self.pbc)
+                q12 = self.cpl.get("dmi_q12")
+                if q12 is not None and np.any(np.asarray(q12)):
+                    # Eq.4 with s != s' ("a third DMI tensor is used to describe the intersublattice
+                    # interaction", D^(s,s') = D^(s',s)): eps = sum_i q12_i . (m x d_i m' + m' x d_i m), whose
+                    # variation gives B^(s) = (2/Ms^(s)) sum_i q12_i x d_i m^(s') -- the intra-sublattice
+                    # expression with the partner's magnetisation (reading S33 for the tensor <-> q_i mapping)
+                    out[T_DMI_INTER] = out[T_DMI_INTER] + fl.dmi_tensor(m[o], p["Ms"], np.asarray(q12, float),
+                                                                        self.cell, self.pbc)
             if terms & T_DMI_HOMO:
                 out[T_DMI_HOMO] = fl.dmi_homogeneous(m[o], p["Ms"], self.cpl.get("d_homo", (0.0, 0.0, 0.0)), s)
         if (terms & T_MEL) and self.elastic is not None:

@@ -267,3 +267,58 @@ def test_P22_bulk_dmi_helix_closed_form_and_interfacial_special_case():
         a = fl.dmi_tensor(mm, Msr, qi, (2e-9, 3e-9, 1e-9), pbc)
         b = fl.dmi_interfacial(mm, Msr, D * np.ones_like(Msr), (2e-9, 3e-9, 1e-9), pbc)
         np.testing.assert_allclose(a, b, atol=1e-12 * np.abs(b).max())
+
+
+def test_P22b_inter_sublattice_dmi_tensor_is_the_gradient_of_eq4():
+    """Eq.4 for s != s': the double sum over (s, s') with D^(1,2) = D^(2,1) is written out on a
+    periodic grid, eps = sum_ijk D_ijk (m1_j d_i m2_k + m2_j d_i m1_k), and differentiated numerically with respect
+    to either sublattice; the oracle's inter-sublattice field, taken through World.field_terms (so the partner
+    wiring and the per-sublattice Ms are pinned too), must be its gradient."""
+    rng = np.random.default_rng(33)
+    grid, cell = (6, 5, 4), (2e-9, 2.5e-9, 1.5e-9)
+    spec = wl.make("c3", grid)
+    spec.cell, spec.pbc, spec.regions, spec.demag = cell, (1, 1, 1), None, False
+    spec.mat = wl.make_mat(2, Ms=np.array([[4e5], [7e5]]), A=1e-11, alpha=0.1)
+    q12 = 1e-3 * rng.standard_normal((3, 3))
+    spec.coupling = wl.default_coupling(latcon=0.35e-9)
+    spec.coupling["dmi_q12"] = q12
+    spec.m = [rng.standard_normal((3, grid[2], grid[1], grid[0])).astype(np.float32) for _ in range(2)]
+    w = World(spec)
+    D = _dijk_from_q(q12)
+    V = float(np.prod(cell))
+
+    def eq4_energy(m1, m2):
+        E = 0.0
+        for i in range(3):
+            ax = 3 - i
+            d1 = (np.roll(m1, -1, axis=ax) - np.roll(m1, 1, axis=ax)) / (2 * cell[i])
+            d2 = (np.roll(m2, -1, axis=ax) - np.roll(m2, 1, axis=ax)) / (2 * cell[i])
+            E += np.einsum("jk,jzyx,kzyx->", D[i], m1, d2) + np.einsum("jk,jzyx,kzyx->", D[i], m2, d1)
+        return V * E
+
+    B = [w.field_terms(s, terms=T_DMI_INTER)[T_DMI_INTER] for s in range(2)]
+    scale = max(np.abs(b).max() for b in B)
+    for _ in range(16):
+        s = int(rng.integers(0, 2))
+        c = int(rng.integers(0, 3))
+        iz, iy, ix = (int(rng.integers(0, k)) for k in (grid[2], grid[1], grid[0]))
+        m0 = w.m[s][c, iz, iy, ix]
+        E = []
+        for sgn in (+1, -1):
+            w.m[s][c, iz, iy, ix] = m0 + sgn * 1e-4
+            E.append(eq4_energy(w.m[0], w.m[1]))
+        w.m[s][c, iz, iy, ix] = m0
+        want = -(E[0] - E[1]) / 2e-4 / (w.p[s]["Ms"][iz, iy, ix] * V)
+        assert abs(B[s][c, iz, iy, ix] - want) < 1e-7 * scale, (s, c)
+    # and the interfacial special case: q12_x = D y^, q12_y = -D x^ equals coupling D_inter = D
+    Dv = 1.3e-3
+    spec2 = spec.copy()
+    spec2.pbc = (0, 1, 0)
+    spec2.coupling["dmi_q12"] = np.array([[0, Dv, 0], [-Dv, 0, 0], [0, 0, 0]], float)
+    spec3 = spec2.copy()
+    spec3.coupling["dmi_q12"] = None
+    spec3.coupling["D_inter"] = Dv
+    for s in range(2):
+        a = World(spec2).field_terms(s, terms=T_DMI_INTER)[T_DMI_INTER]
+        b = World(spec3).field_terms(s, terms=T_DMI_INTER)[T_DMI_INTER]
+        np.testing.assert_allclose(a, b, atol=1e-12 * np.abs(b).max())
