@@ -182,6 +182,24 @@ int mmx_set_current(mmx_world* w, const double J[3]);  /* Zhang-Li current densi
  * the interfacial term of mmx_material.D under the same term bit MMX_T_DMI.  Interfacial D equals
  * q_x = D y^, q_y = -D x^; bulk DMI eps = D m.(curl m) equals q_i = -D e_i.  q = NULL clears it. */
 int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]);
+/* sublattice = MMX_DMI_INTER: the third tensor of Eq.4, "used to describe the intersublattice interaction",
+ * D^(s,s') = D^(s',s): B^(s) = (2/Ms^(s)) sum_i q_i x d_i m^(s'), added to the interfacial mmx_coupling.D_inter
+ * under the term bit MMX_T_DMI_INTER (two-sublattice worlds). */
+#define MMX_DMI_INTER (-1)
+
+/* Slonczewski spin-transfer torque ("as formulated by ... Slonczewski [29], implemented in the same way
+ * as in mumax3"; reading S37).  A current density jz through the free layer (thickness d), polarised along
+ * the fixed-layer direction mp, adds in Gilbert form  gamma beta [eps m x (mp x m) - eps' m x mp],
+ * beta = hbar jz/(e Ms d), eps = P L^2/((L^2 + 1) + (L^2 - 1) m.mp), P = mmx_material.pol; the explicit torque is
+ * gamma beta/(1 + alpha^2) [(eps + alpha eps') m x (mp x m) - (eps' - alpha eps) m x mp].  NULL (or jz = 0) clears. */
+typedef struct mmx_slonczewski {
+  double jz;         /* current density through the layer, A/m^2                        */
+  double mp[3];      /* fixed-layer polarisation direction (normalised by the library)  */
+  double lambda;     /* Slonczewski Lambda (>= 1; 1: no angular dependence, eps = P/2)  */
+  double eps_prime;  /* secondary (field-like) spin-torque parameter eps'               */
+  double thickness;  /* free-layer thickness d, m; <= 0: Nz * cellsize[2]               */
+} mmx_slonczewski;
+int mmx_set_slonczewski(mmx_world* w, const mmx_slonczewski* s);
 /* Enable elastodynamics (adds the fields U, V to the integrated state); NULL disables. */
 int mmx_set_elastic(mmx_world* w, const mmx_elastic* e);
 /* Switch the magnetostatic term on/off for stepping (default on once the kernel exists). */

@@ -228,8 +228,9 @@ def slonczewski_torque(m, Ms, alpha, gamma, pol, jz, mp, lam, eps_prime, thickne
         eps = P Lambda^2 / ((Lambda^2 + 1) + (Lambda^2 - 1) (m . m_p))
     to  dm/dt = -gamma m x B + alpha m x dm/dt + T.  Solving for dm/dt (as for Eq.2) gives the explicit torque
         tau_SL = gamma beta / (1 + alpha^2) [ (eps + alpha eps') m x (m_p x m) - (eps' - alpha eps) m x m_p ].
-    m_p [3] unit vector; returns 1/s."""
-    mpv = np.asarray(mp, float).reshape(3, 1, 1, 1) * np.ones_like(m)
+    m_p [3]: direction of the fixed layer (normalised here); returns 1/s."""
+    mp = np.asarray(mp, float)
+    mpv = (mp / np.sqrt((mp * mp).sum())).reshape(3, 1, 1, 1) * np.ones_like(m)   # m_p is a direction
     beta = HBAR * jz / (Q_E * thickness) * _inv(Ms)
     l2 = lam * lam
     eps = pol * l2 / ((l2 + 1.0) + (l2 - 1.0) * (m * mpv).sum(axis=0))

@@ -19,6 +19,7 @@ T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0, T_DMI_INTER, 
     1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1024)
 T_ALL = 2047
 F_M0, F_M1, F_U, F_V = 0, 1, 2, 3
+DMI_INTER = -1
 RK4, DP45, HEUN12, BS23, CK45, RKF45 = 0, 1, 2, 3, 4, 5
 FACES = {"x-": 0, "x+": 1, "y-": 2, "y+": 3, "z-": 4, "z+": 5}
 
@@ -42,6 +43,11 @@ class Material(C.Structure):
 class Coupling(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("A0", "A12", "latcon", "D_inter", "scale_A11", "scale_A12")] + [
         ("d_homo", C.c_double * 3)]
+
+
+class Slonczewski(C.Structure):
+    _fields_ = [("jz", C.c_double), ("mp", C.c_double * 3), ("lambda_", C.c_double), ("eps_prime", C.c_double),
+                ("thickness", C.c_double)]
 
 
 class Elastic(C.Structure):
@@ -77,6 +83,7 @@ PROTOTYPES = {
     "mmx_set_bext": (C.c_int, [_W, _D3]),
     "mmx_set_current": (C.c_int, [_W, _D3]),
     "mmx_set_dmi_tensor": (C.c_int, [_W, C.c_int, C.POINTER(C.c_double)]),
+    "mmx_set_slonczewski": (C.c_int, [_W, C.POINTER(Slonczewski)]),
     "mmx_set_elastic": (C.c_int, [_W, C.POINTER(Elastic)]),
     "mmx_enable_demag": (C.c_int, [_W, C.c_int]),
     "mmx_set_state": (C.c_int, [_W, C.c_int, C.c_void_p, C.c_int]),
@@ -232,6 +239,12 @@ class World:
         flat = [float(x) for x in np.asarray(q, dtype=np.float64).reshape(9)]
         _check(self.lib.mmx_set_dmi_tensor(self.h, int(sublattice), _arr(C.c_double, flat)))
 
+    def set_slonczewski(self, jz=0.0, mp=(0.0, 0.0, 1.0), thickness=0.0, eps_prime=0.0, **kw):
+        """Slonczewski torque parameters (keyword `lambda`: Slonczewski Lambda, default 1); jz = 0 clears."""
+        sl = Slonczewski(float(jz), (C.c_double * 3)(*[float(x) for x in mp]), float(kw.get("lambda", 1.0)),
+                         float(eps_prime), float(thickness or 0.0))
+        _check(self.lib.mmx_set_slonczewski(self.h, C.byref(sl)))
+
     def set_current(self, J):
         _check(self.lib.mmx_set_current(self.h, _arr(C.c_double, [float(x) for x in J])))
 
@@ -371,10 +384,16 @@ class World:
                 w.set_material(s, r, **kw)
         cpl = dict(spec.coupling)
         dmi_q = cpl.pop("dmi_q", None)
+        dmi_q12 = cpl.pop("dmi_q12", None)
+        sl = cpl.pop("slonczewski", None)
         w.set_coupling(**cpl)
         if dmi_q is not None:
             for s in range(spec.S):
                 w.set_dmi_tensor(s, np.asarray(dmi_q)[s])
+        if dmi_q12 is not None:
+            w.set_dmi_tensor(DMI_INTER, np.asarray(dmi_q12))
+        if sl:
+            w.set_slonczewski(**sl)
         w.set_bext(spec.bext)
         w.set_current(spec.J)
         if spec.elastic is not None:

@@ -162,6 +162,7 @@ int upload_params(mmx_world* w) {
       p[MP_B2] = (float)m.B2;
       p[MP_ZLB] = (float)(MU_B * m.pol * iMs / (Q_E * (1.0 + m.xi * m.xi)));
       p[MP_XI] = (float)m.xi;
+      p[MP_POL] = (float)m.pol;
     }
   MMX_CUDA(cudaMemcpyAsync(w->d_mat, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, w->stream));
   MMX_CUDA(cudaStreamSynchronize(w->stream));  // tab goes out of scope
@@ -250,8 +251,21 @@ void fill_local(const mmx_world* w, LocalArgs& a, unsigned terms) {
   a.Dinter = (float)w->cpl.D_inter;
   for (int k = 0; k < 3; ++k) a.dhomo[k] = (float)w->cpl.d_homo[k];
   a.has_dmiq = w->has_dmiq ? 1 : 0;
-  for (int s = 0; s < 2; ++s)
-    for (int k = 0; k < 9; ++k) a.dmiq[s][k / 3][k % 3] = (float)w->dmiq[s][k];
+  a.has_dmiq12 = 0;
+  for (int s = 0; s < 3; ++s)
+    for (int k = 0; k < 9; ++k) {
+      a.dmiq[s][k / 3][k % 3] = (float)w->dmiq[s][k];
+      if (s == 2 && w->dmiq[s][k] != 0.0) a.has_dmiq12 = 1;
+    }
+  a.has_sl = w->sl.jz != 0.0 ? 1 : 0;
+  {
+    const double HBAR = 1.054571817e-34;
+    const double d = w->sl.thickness > 0 ? w->sl.thickness : w->grid[2] * w->cell[2];
+    a.sl_beta = (float)(HBAR * w->sl.jz / (Q_E * d));
+    for (int k = 0; k < 3; ++k) a.sl_mp[k] = (float)w->sl.mp[k];
+    a.sl_l2 = (float)(w->sl.lambda * w->sl.lambda);
+    a.sl_epsp = (float)w->sl.eps_prime;
+  }
   a.terms = terms;
   a.has_J = (w->J[0] != 0.0 || w->J[1] != 0.0 || w->J[2] != 0.0) ? 1 : 0;
   a.bdemag = (terms & MMX_T_DEMAG) ? w->bdemag : nullptr;
@@ -574,8 +588,9 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
     else { cudaGetLastError(); w->stream = nullptr; }
   }
   w->has_dmiq = false;
-  for (int s = 0; s < 2; ++s)
+  for (int s = 0; s < 3; ++s)
     for (int k = 0; k < 9; ++k) w->dmiq[s][k] = 0.0;
+  memset(&w->sl, 0, sizeof(w->sl));
   w->n_tmaps = 0;
   w->step_graph = nullptr; w->graph_method = -1; w->graph_epoch = -1; w->cfg_epoch = 0; w->graph_launches = 0;
   w->use_graphs = getenv("MMX_NO_GRAPH") == nullptr;
@@ -711,11 +726,32 @@ int mmx_set_current(mmx_world* w, const double J[3]) {
 
 int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]) {
   if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
-  if (sublattice < 0 || sublattice >= w->S) return mmx_fail(MMX_EINVAL, "sublattice %d out of range", sublattice);
+  if (sublattice == MMX_DMI_INTER) {
+    if (w->S != 2) return mmx_fail(MMX_EINVAL, "the inter-sublattice DMI tensor needs two sublattices");
+    sublattice = 2;
+  } else if (sublattice < 0 || sublattice >= w->S) {
+    return mmx_fail(MMX_EINVAL, "sublattice %d out of range", sublattice);
+  }
   for (int k = 0; k < 9; ++k) w->dmiq[sublattice][k] = q ? q[k] : 0.0;
   w->has_dmiq = false;
-  for (int s = 0; s < 2; ++s)
+  for (int s = 0; s < 3; ++s)
     for (int k = 0; k < 9; ++k) w->has_dmiq = w->has_dmiq || w->dmiq[s][k] != 0.0;
+  w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
+  return MMX_OK;
+}
+
+int mmx_set_slonczewski(mmx_world* w, const mmx_slonczewski* sl) {
+  if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
+  if (!sl) {
+    memset(&w->sl, 0, sizeof(w->sl));
+  } else {
+    const double n = sqrt(sl->mp[0] * sl->mp[0] + sl->mp[1] * sl->mp[1] + sl->mp[2] * sl->mp[2]);
+    if (sl->jz != 0.0 && !(n > 0)) return mmx_fail(MMX_EINVAL, "Slonczewski torque needs a fixed-layer direction mp");
+    if (sl->jz != 0.0 && !(sl->lambda >= 1.0)) return mmx_fail(MMX_EINVAL, "Slonczewski Lambda must be >= 1");
+    w->sl = *sl;
+    for (int k = 0; k < 3; ++k) w->sl.mp[k] = n > 0 ? sl->mp[k] / n : 0.0;
+  }
   w->k1_valid = false;
   w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;

@@ -162,6 +162,11 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
                     if (axis == 0) { B.x = fmaf(wd, on.z, B.x); B.z = fmaf(-wd, on.x, B.z); }
                     else { B.y = fmaf(wd, on.z, B.y); B.z = fmaf(-wd, on.y, B.z); }
                   }
+                  if (a.has_dmiq12 && (a.terms & MMX_T_DMI_INTER)) {
+                    // inter-sublattice tensor of Eq.4: B_c += d /(Ms_c h_i) q12_i x m'_n
+                    const V3 qv = v3(a.dmiq[2][axis][0], a.dmiq[2][axis][1], a.dmiq[2][axis][2]);
+                    B = fma3(iMs * a.inv_h[axis] * d, cross(qv, on), B);
+                  }
                 }
               }
             }
@@ -217,6 +222,16 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
           const float inv = -1.f / (1.f + alpha * alpha);
           tau = fma3(inv * (1.f + xi * alpha), mxmxa, tau);
           tau = fma3(inv * (xi - alpha), mxa, tau);
+        }
+        if (a.has_sl) {
+          // Slonczewski torque (reading S37): gamma beta/(1+alpha^2) [(eps + alpha eps') m x (p x m) + (eps' - alpha eps) p x m]
+          const V3 pv = v3(a.sl_mp[0], a.sl_mp[1], a.sl_mp[2]);
+          const float eps = P[MP_POL] * a.sl_l2 / ((a.sl_l2 + 1.f) + (a.sl_l2 - 1.f) * dot(m, pv));
+          const V3 pxm = cross(pv, m);
+          const V3 mxpxm = cross(m, pxm);
+          const float pref = P[MP_LLG] * a.sl_beta * iMs;
+          tau = fma3(pref * (eps + alpha * a.sl_epsp), mxpxm, tau);
+          tau = fma3(pref * (a.sl_epsp - alpha * eps), pxm, tau);
         }
       }
       if (a.heff_out) { st3(a.heff_out, N, i, B); continue; }
@@ -952,7 +967,8 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   const unsigned blocks = (unsigned)((N + 255) / 256);
   const bool reg = w->nreg > 1;
   ProfScope ps(w, PK_LOCAL);
-  bool uniform = !reg && (w->grid[0] % 4) == 0 && !a.has_dmiq;  // (the general DMI tensor lives in k_local only)
+  // (the general DMI tensors and the Slonczewski torque live in the general kernel k_local only)
+  bool uniform = !reg && (w->grid[0] % 4) == 0 && !a.has_dmiq && !a.has_sl;
   for (int s = 0; s < w->S && uniform; ++s) uniform = w->mats[(size_t)s * w->nreg].Ms > 0;
   const bool open_all = !a.per[0] && !a.per[1] && !a.per[2];
   if (uniform && w->S == 1 && open_all) {

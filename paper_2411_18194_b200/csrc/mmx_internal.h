@@ -20,7 +20,7 @@ enum {
   MP_KU2 /* 2Ku1/Ms */, MP_UX, MP_UY, MP_UZ,
   MP_KC2 /* 2Kc1/Ms */, MP_C1X, MP_C1Y, MP_C1Z, MP_C2X, MP_C2Y, MP_C2Z, MP_C3X, MP_C3Y, MP_C3Z,
   MP_MEL1 /* 2B1/Ms */, MP_MEL2 /* 2B2/Ms */, MP_B1, MP_B2,
-  MP_ZLB /* mu_B pol / (e Ms (1+xi^2)) */, MP_XI,
+  MP_ZLB /* mu_B pol / (e Ms (1+xi^2)) */, MP_XI, MP_POL,
   MP_COUNT
 };
 
@@ -63,8 +63,13 @@ struct LocalArgs {
   const float* mat;      // [S][nreg][MMX_MATW]
   float scaleA11, scaleA12, A12, a0pref, Dinter;
   float dhomo[3];        // DMI vector of Eq.6, J/m^3
-  float dmiq[2][3][3];   // general DMI tensor of Eq.4 as per-axis vectors q_i per sublattice, J/m^2
-  int has_dmiq;
+  float dmiq[3][3][3];   // general DMI tensor of Eq.4 as per-axis vectors q_i: sublattice 0, 1, inter-sublattice; J/m^2
+  int has_dmiq;          // any tensor set (routes the world to the general kernel)
+  int has_dmiq12;        // the inter-sublattice one
+  // Slonczewski torque (reading S37)
+  int has_sl;
+  float sl_beta;         // hbar jz / (e d): times 1/Ms gives beta in tesla
+  float sl_mp[3], sl_l2, sl_epsp;
   float bext[3], J[3];
   unsigned terms;
   int has_J;
@@ -162,8 +167,9 @@ struct mmx_world {
   bool mat_dirty;
   mmx_coupling cpl;
   double bext[3], J[3];
-  double dmiq[2][9];   // general DMI tensor (mmx_set_dmi_tensor), zero = none
+  double dmiq[3][9];   // general DMI tensors (mmx_set_dmi_tensor): sublattice 0, 1, inter-sublattice; zero = none
   bool has_dmiq;
+  mmx_slonczewski sl;  // jz = 0: off
   bool has_elastic;
   mmx_elastic el;
   bool use_demag;

@@ -1,0 +1,117 @@
+"""GPU parity of the SURVEY 8(f) "NEXT" rows against the fp64 oracle (through the C-ABI): Slonczewski torque
+(reading S37), inter-sublattice general DMI tensor (Eq.4, s != s').  Same bars as everywhere: per-cell relative field /
+torque error 1e-5, max |delta m| 1e-4 after a fixed-step trajectory."""
+import numpy as np
+import pytest
+
+import paper_2411_18194_b200 as mmx
+import workloads as wl
+from oracle import constants as oc
+from gpu_util import FIELD_TOL, TRAJ_TOL, field_err, max_dm, pair
+from test_gpu_fields import _rich_spec
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("name,grid", [("c1", (64, 16, 1)), ("c4", (20, 12, 6)), ("c3", (48, 24, 1))])
+def test_slonczewski_torque_and_trajectory(name, grid):
+    """P:L39, L110; reading S37.  Torque of every sublattice with the spin-transfer term switched on (uniform
+    worlds, a world with 1669-grain-style regions, 3-D), against the oracle; the term must matter; 30 DP45 steps."""
+    spec = _rich_spec(name, grid, seed=5)
+    spec.mat["pol"][:] = 0.56
+    sl = dict(jz=-4.0e11, mp=(0.3, -0.2, 0.93), eps_prime=0.02, thickness=3e-9)
+    sl["lambda"] = 1.4
+    spec.coupling["slonczewski"] = sl
+    g, o = pair(spec)
+    plain = spec.copy()
+    plain.coupling["slonczewski"] = None
+    from gpu_util import pair_oracle
+    o0 = pair_oracle(plain)
+    for s in range(spec.S):
+        ref = o.torque(s)
+        assert field_err(o0.torque(s), ref) > 1e-3            # the spin-transfer torque is a visible part of tau
+        assert field_err(g.eval_torque(s), ref) < FIELD_TOL, (name, s)
+    dt = spec.integrator["dt"]
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=30)
+    o.step_dp45_fixed(dt, 30)
+    for s in range(spec.S):
+        assert max_dm(g.get_state(mmx.F_M0 + s), o.m[s]) <= TRAJ_TOL
+    # clearing it restores the plain torque
+    g.set_slonczewski(jz=0.0)
+    g.set_state(mmx.F_M0, np.ascontiguousarray(spec.m[0], dtype=np.float32))
+    if spec.S == 2:
+        g.set_state(mmx.F_M1, np.ascontiguousarray(spec.m[1], dtype=np.float32))
+    assert field_err(g.eval_torque(0), o0.torque(0)) < FIELD_TOL
+    g.destroy()
+
+
+def test_slonczewski_switching_closed_form_on_the_cuda_path():
+    """P23 end to end on the GPU: macrospin, fixed layer along z, Lambda = 1:
+    m_z(t) = tanh(gamma (alpha (B + beta eps') + beta eps) t /(1 + alpha^2) + atanh m_z(0))."""
+    HBAR, QE, GAMMA = 1.054571817e-34, 1.602176634e-19, 1.7595e11
+    Ms, alpha, P, d, B, epsp, jz = 8.0e5, 0.02, 0.4, 2e-9, 0.2, 0.05, -6.0e11
+    spec = wl.make("c1", (4, 1, 1))
+    spec.demag = False
+    spec.mat["alpha"][:] = alpha
+    spec.mat["pol"][:] = P
+    spec.mat["A"][:] = 0.0
+    spec.bext = (0.0, 0.0, B)
+    m0 = np.array([np.sin(0.6), 0.0, np.cos(0.6)])
+    spec.m = [np.tile(m0.reshape(3, 1, 1, 1), (1, 1, 1, 4)).astype(np.float32)]
+    sl = dict(jz=jz, mp=(0.0, 0.0, 1.0), eps_prime=epsp, thickness=d)
+    sl["lambda"] = 1.0
+    spec.coupling["slonczewski"] = sl
+    g = mmx.World.from_spec(spec)
+    dt, n = 2e-14, 2000
+    g.step_rk4(dt, n)
+    beta = HBAR * jz / (QE * Ms * d)
+    rate = GAMMA * (alpha * (B + beta * epsp) + beta * P / 2) / (1 + alpha ** 2)
+    mz = np.tanh(rate * n * dt + np.arctanh(float(spec.m[0][2, 0, 0, 0])))
+    assert rate < 0                                             # beyond the switching current: m_z falls
+    got = g.get_state(mmx.F_M0)[2, 0, 0, :]
+    assert np.abs(got - mz).max() < 2e-5, (got, mz)
+    g.destroy()
+
+
+@pytest.mark.parametrize("grid,pbc", [((48, 24, 1), (0, 0, 0)), ((32, 16, 1), (2, 2, 0)), ((20, 12, 4), (0, 0, 0))])
+def test_inter_sublattice_dmi_tensor(grid, pbc):
+    """Eq.4, the third tensor "used to describe the intersublattice interaction": per-sublattice field under
+    MMX_T_DMI_INTER (added to the interfacial D_inter), total field, torque, energy and a 20-step trajectory on a
+    two-sublattice world with regions (c3 recipe), open / periodic / 3-D."""
+    spec = _rich_spec("c3", grid, seed=29)
+    spec.pbc = pbc
+    rng = np.random.default_rng(37)
+    spec.coupling["dmi_q12"] = 1e-3 * rng.standard_normal((3, 3))
+    spec.coupling["dmi_q"] = 0.5e-3 * rng.standard_normal((2, 3, 3))
+    g, o = pair(spec)
+    plain = spec.copy()
+    plain.coupling["dmi_q12"] = None
+    from gpu_util import pair_oracle
+    o0 = pair_oracle(plain)
+    for s in range(2):
+        ref = o.field_terms(s, terms=oc.T_DMI_INTER)[oc.T_DMI_INTER]
+        assert field_err(o0.field_terms(s, terms=oc.T_DMI_INTER)[oc.T_DMI_INTER], ref) > 1e-2   # the tensor part matters
+        assert field_err(g.eval_heff(s, mmx.T_DMI_INTER), ref) < FIELD_TOL, s
+        assert field_err(g.eval_heff(s, mmx.T_ALL), o.heff(s)) < FIELD_TOL, s
+        assert field_err(g.eval_torque(s), o.torque(s)) < FIELD_TOL, s
+    Eg, Eo = g.energy(mmx.T_DMI_INTER), o.energy(oc.T_DMI_INTER)
+    assert abs(Eg - Eo) < 1e-5 * abs(Eo)
+    dt = spec.integrator["dt"]
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=20)
+    o.step_dp45_fixed(dt, 20)
+    for s in range(2):
+        assert max_dm(g.get_state(mmx.F_M0 + s), o.m[s]) <= TRAJ_TOL
+    g.destroy()
+
+
+def test_argument_errors_of_the_new_setters():
+    spec = wl.make("c1", (8, 4, 1))
+    g = mmx.World.from_spec(spec, demag=False)
+    with pytest.raises(mmx.MmxError):
+        g.set_dmi_tensor(mmx.DMI_INTER, np.ones((3, 3)))       # one sublattice: no inter-sublattice tensor
+    with pytest.raises(mmx.MmxError):
+        g.set_slonczewski(jz=1e11, mp=(0, 0, 0))               # no fixed-layer direction
+    kw = {"lambda": 0.5}
+    with pytest.raises(mmx.MmxError):
+        g.set_slonczewski(jz=1e11, mp=(0, 0, 1), **kw)          # Lambda < 1
+    g.destroy()
