@@ -185,9 +185,15 @@ def cross(a, b):
     return np.stack([a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]])
 
 
-def llg_torque(m, B, alpha, gamma):
-    """Eq.2: tau = -gamma/(1+alpha^2) [ m x B + alpha m x (m x B) ]   (1/s)."""
+def llg_torque(m, B, alpha, gamma, precession=True):
+    """Eq.2: tau = -gamma/(1+alpha^2) [ m x B + alpha m x (m x B) ]   (1/s).
+    precession=False drops the m x B term: the damping-only torque that a relaxation follows ("after
+    letting a non-collinear antiferromagnet relax from a random state"; the paper does not say how -- reading
+    S39: as mumax3's relax(), the precession term is switched off and the damping term is integrated with the
+    adaptive scheme until the torque falls below a threshold)."""
     mxB = cross(m, B)
+    if not precession:
+        return (-gamma / (1.0 + alpha * alpha))[None] * (alpha[None] * cross(m, mxB))
     return (-gamma / (1.0 + alpha * alpha))[None] * (mxB + alpha[None] * cross(m, mxB))
 
 

@@ -52,6 +52,7 @@ class World:
         self._spectrum = None
         self._k1 = None
         self._k1_tab = None
+        self.precession = True   # False: relaxation mode (reading S39), torque() drops the m x B term
         self.V = self.cell[0] * self.cell[1] * self.cell[2]
 
     # ------------------------------------------------------------------ demag
@@ -135,7 +136,7 @@ class World:
         """Eq.1-2 (+ Zhang-Li when J != 0): tau for sublattice s, 1/s."""
         m = self.m if m is None else m
         p = self.p[s]
-        tau = fl.llg_torque(m[s], self.heff(s, m, u, terms, b_demag), p["alpha"], p["gamma"])
+        tau = fl.llg_torque(m[s], self.heff(s, m, u, terms, b_demag), p["alpha"], p["gamma"], self.precession)
         if any(j != 0.0 for j in self.J):
             tau = tau + fl.zhang_li_torque(m[s], p["Ms"], p["alpha"], p["pol"], p["xi"], self.J,
                                            self.cell, self.pbc)
@@ -228,8 +229,18 @@ class World:
         k = self.rhs(self.get_state(), self.t)
         return self.mag_norm(k)
 
+    def relax(self, torque_stop, tab=rk.DP45, tol=1e-5, max_attempts=100000):
+        """Relaxation (reading S39): damping-only torque, adaptive steps, until max_c |tau_c| < torque_stop [1/s].
+        The spin-transfer torques stay as they are (callers relax without currents).  Time is not advanced."""
+        t0, self.precession, self._k1 = self.t, False, None
+        try:
+            out = self.run_adaptive(tab, tol, max_attempts=max_attempts, torque_stop=torque_stop)
+        finally:
+            self.precession, self._k1, self.t = True, None, t0
+        return out
+
     def run_adaptive(self, tab=rk.DP45, tol=1e-5, dt0=None, nsteps=None, t_end=None, max_attempts=100000,
-                     log=None, dt_max=None):
+                     log=None, dt_max=None, torque_stop=None):
         """Adaptive stepping with an embedded pair (controller S21; the step-size exponent is
         1/convergence order).  Returns dict(accepted, rejected, dt, t, last_err); `log`, when a list,
         receives one (dt, err, accepted) tuple per attempt.  dt_max: no step above it is proposed
@@ -246,6 +257,8 @@ class World:
             if nsteps is not None and acc >= nsteps:
                 break
             if t_end is not None and self.t >= t_end:
+                break
+            if torque_stop is not None and self.mag_norm(self._k1) < torque_stop:
                 break
             if t_end is not None and self.t + dt > t_end:
                 dt = t_end - self.t

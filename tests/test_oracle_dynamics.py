@@ -332,3 +332,35 @@ def test_slonczewski_angular_dependence():
         m = one((np.sin(th), 0, sgn * np.cos(th)))
         tau = fl.slonczewski_torque(m, arr(Ms), arr(0.0), arr(GAMMA), arr(P), jz, (0, 0, 1), lam, 0.0, d)
         np.testing.assert_allclose(np.sqrt((tau ** 2).sum()) / np.sin(th), GAMMA * abs(beta) * eps, rtol=1e-5)
+
+
+def test_P24_relaxation_closed_form_and_energy_descent():
+    """P24 (pins reading S39).  Damping-only torque of a macrospin in B z^: the azimuth stays put and
+    m_z(t) = tanh(alpha gamma B t/(1 + alpha^2) + atanh m_z(0)) -- the damping part of P7 with the precession gone.
+    On an exchange + anisotropy + demag film the relaxation lowers the energy monotonically and ends in a state
+    whose FULL LLG torque is below the same threshold times sqrt(1 + alpha^2)/alpha (|m x B| is common to both)."""
+    alpha, B = 0.3, 0.7
+    w = _macrospin(alpha, B, (0.48, 0.36, 0.8))
+    w.precession = False
+    dt, n = 1e-13, 300
+    w.step_rk4(dt, n)
+    mz = np.tanh(alpha * GAMMA * B * n * dt / (1 + alpha ** 2) + np.arctanh(0.8))
+    got = w.m[0][:, 0, 0, 0]
+    assert abs(got[2] - mz) < 1e-9
+    assert abs(np.arctan2(got[1], got[0]) - np.arctan2(0.36, 0.48)) < 1e-12
+    spec = wl.make("c2", (16, 16, 1))
+    o = World(spec)
+    E = [o.energy(T_ALL)]
+    o.precession = False
+    for _ in range(40):
+        o.run_adaptive(rk.DP45, 1e-5, nsteps=3)
+        E.append(o.energy(T_ALL))
+    assert all(b <= a + 1e-9 * abs(a) for a, b in zip(E, E[1:]))
+    o.precession = True
+    o2 = World(spec)
+    a = float(spec.mat["alpha"][0, 0])
+    stop = 1e-3 * GAMMA   # 1 mT in torque units
+    st = o2.relax(stop)
+    assert st["accepted"] > 0 and o2.t == 0.0 and o2.precession
+    assert o2.max_torque() < stop * np.sqrt(1 + a * a) / a * 1.0001
+    assert o2.energy(T_ALL) < E[0]
