@@ -270,6 +270,12 @@ int mmx_step_rk4(mmx_world* w, double dt, long long nsteps);
  *   - MMX_ENAN: a NaN/Inf reached the error or torque reduction; the attempt is not accepted, the
  *     accepted state and time are left as they were, stepping stops. */
 int mmx_step_rk45(mmx_world* w, const mmx_rk_opts* opts, mmx_rk_stats* stats);
+
+/* Relaxation ("after letting a non-collinear antiferromagnet relax from a random state"; DESIGN.md reading
+ * S39): the precession term m x B of Eq.2 is dropped and the damping term -gamma alpha/(1+alpha^2) m x (m x B) is
+ * integrated with adaptive Dormand-Prince steps (tolerance tol, <= 0: 1e-5) until max_c |tau_c| < torque_stop [1/s]
+ * or max_attempts (<= 0: 1e6) attempts were made.  The simulation time is left where it was.  stats may be NULL. */
+int mmx_relax(mmx_world* w, double torque_stop, double tol, long long max_attempts, mmx_rk_stats* stats);
 /* Error estimates of the most recent attempted steps (newest last); returns the number
  * written through *n_out (at most n). */
 int mmx_get_err_history(mmx_world* w, double* host_out, int n, int* n_out);

@@ -102,6 +102,7 @@ PROTOTYPES = {
     "mmx_max_torque": (C.c_int, [_W, _D3]),
     "mmx_step_rk4": (C.c_int, [_W, C.c_double, C.c_longlong]),
     "mmx_step_rk45": (C.c_int, [_W, C.POINTER(RkOpts), C.POINTER(RkStats)]),
+    "mmx_relax": (C.c_int, [_W, C.c_double, C.c_double, C.c_longlong, C.POINTER(RkStats)]),
     "mmx_get_err_history": (C.c_int, [_W, _D3, C.c_int, _I3]),
     "mmx_profile_enable": (C.c_int, [_W, C.c_int]),
     "mmx_profile_read": (C.c_int, [_W, _D3, C.POINTER(C.c_longlong), C.c_int]),
@@ -335,6 +336,11 @@ class World:
                    float(torque_stop), int(max_attempts), float(dt_max))
         st = RkStats()
         _check(self.lib.mmx_step_rk45(self.h, C.byref(o), C.byref(st)))
+        return {k: getattr(st, k) for k, _ in RkStats._fields_}
+
+    def relax(self, torque_stop, tol=1e-5, max_attempts=0):
+        st = RkStats()
+        _check(self.lib.mmx_relax(self.h, float(torque_stop), float(tol), int(max_attempts), C.byref(st)))
         return {k: getattr(st, k) for k, _ in RkStats._fields_}
 
     def get_err_history(self, n=4096):

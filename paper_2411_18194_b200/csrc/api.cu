@@ -268,6 +268,7 @@ void fill_local(const mmx_world* w, LocalArgs& a, unsigned terms) {
   }
   a.terms = terms;
   a.has_J = (w->J[0] != 0.0 || w->J[1] != 0.0 || w->J[2] != 0.0) ? 1 : 0;
+  a.relax = w->relax_mode ? 1 : 0;
   a.bdemag = (terms & MMX_T_DEMAG) ? w->bdemag : nullptr;
   a.strain = (terms & MMX_T_MEL) ? w->strain : nullptr;
   a.ctrl = w->d_ctrl;
@@ -591,6 +592,7 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
   for (int s = 0; s < 3; ++s)
     for (int k = 0; k < 9; ++k) w->dmiq[s][k] = 0.0;
   memset(&w->sl, 0, sizeof(w->sl));
+  w->relax_mode = false;
   w->n_tmaps = 0;
   w->step_graph = nullptr; w->graph_method = -1; w->graph_epoch = -1; w->cfg_epoch = 0; w->graph_launches = 0;
   w->use_graphs = getenv("MMX_NO_GRAPH") == nullptr;
@@ -745,6 +747,7 @@ int mmx_set_slonczewski(mmx_world* w, const mmx_slonczewski* sl) {
   if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
   if (!sl) {
     memset(&w->sl, 0, sizeof(w->sl));
+  w->relax_mode = false;
   } else {
     const double n = sqrt(sl->mp[0] * sl->mp[0] + sl->mp[1] * sl->mp[1] + sl->mp[2] * sl->mp[2]);
     if (sl->jz != 0.0 && !(n > 0)) return mmx_fail(MMX_EINVAL, "Slonczewski torque needs a fixed-layer direction mp");
@@ -1042,6 +1045,26 @@ int mmx_step_rk45(mmx_world* w, const mmx_rk_opts* opts, mmx_rk_stats* stats) {
   if (opts->nsteps <= 0 && opts->t_end <= 0 && opts->torque_stop <= 0 && opts->max_attempts <= 0)
     return mmx_fail(MMX_EINVAL, "no stopping criterion");
   return run_steps(w, opts, stats);
+}
+
+int mmx_relax(mmx_world* w, double torque_stop, double tol, long long max_attempts, mmx_rk_stats* stats) {
+  if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
+  if (!(torque_stop > 0)) return mmx_fail(MMX_EINVAL, "mmx_relax needs torque_stop > 0");
+  double t0 = 0;
+  if (int rc = mmx_get_time(w, &t0)) return rc;
+  mmx_rk_opts o;
+  memset(&o, 0, sizeof(o));
+  o.method = MMX_DP45; o.tol = tol; o.torque_stop = torque_stop; o.max_attempts = max_attempts;
+  w->relax_mode = true;
+  w->k1_valid = false;
+  w->cfg_epoch++;  // the local kernels' arguments change: the captured step graph is stale
+  int rc = run_steps(w, &o, stats);
+  w->relax_mode = false;
+  w->k1_valid = false;
+  w->cfg_epoch++;
+  const int rc2 = mmx_set_time(w, t0);
+  if (stats) stats->t = t0;
+  return rc ? rc : rc2;
 }
 
 int mmx_get_err_history(mmx_world* w, double* host_out, int n, int* n_out) {

@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
         const V3 mxB = cross(m, B);
         const V3 mxmxB = cross(m, mxB);
         const float alpha = P[MP_ALPHA];
-        tau = (-P[MP_LLG]) * fma3(alpha, mxmxB, mxB);
+        tau = a.relax ? (-P[MP_LLG] * alpha) * mxmxB : (-P[MP_LLG]) * fma3(alpha, mxmxB, mxB);
         if (a.has_J) {
           // tau_ZL = -(1+alpha^2)^-1 [ (1 + xi alpha) m x (m x dm) + (xi - alpha) m x dm ]
           const float xi = P[MP_XI];
@@ -489,7 +489,7 @@ __global__ void __launch_bounds__(MMX_L4_BLOCK, 2) k_local4(LocalArgs a) {
         B.c[e] = Bc;
         const V3 mxB = cross(m, Bc);
         const V3 mxmxB = cross(m, mxB);
-        V3 t = (-llg) * fma3(alpha, mxmxB, mxB);
+        V3 t = a.relax ? (-llg * alpha) * mxmxB : (-llg) * fma3(alpha, mxmxB, mxB);
         if (a.has_J) {
           const V3 mxa = cross(m, dm.c[e]);
           const V3 mxmxa = cross(m, mxa);
@@ -739,7 +739,7 @@ __global__ void __launch_bounds__(LT_NT, 3) k_local_t(LocalArgs a, const __grid_
       B.c[e] = Bc;
       const V3 mxB = cross(m, Bc);
       const V3 mxmxB = cross(m, mxB);
-      V3 t = (-llg) * fma3(alpha, mxmxB, mxB);
+      V3 t = a.relax ? (-llg * alpha) * mxmxB : (-llg) * fma3(alpha, mxmxB, mxB);
       if (a.has_J) {
         const V3 mxa = cross(m, dm.c[e]);
         const V3 mxmxa = cross(m, mxa);

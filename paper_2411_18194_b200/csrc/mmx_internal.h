@@ -73,6 +73,7 @@ struct LocalArgs {
   float bext[3], J[3];
   unsigned terms;
   int has_J;
+  int relax;             // 1: damping-only torque (mmx_relax, reading S39)
   // inputs.  A "sel pair" p[2] is indexed with ctrl->sel inside the kernel.
   const float* yin[2];     // stage state [nvec][3][N]
   const float* bdemag;     // [3][N] or null
@@ -170,6 +171,7 @@ struct mmx_world {
   double dmiq[3][9];   // general DMI tensors (mmx_set_dmi_tensor): sublattice 0, 1, inter-sublattice; zero = none
   bool has_dmiq;
   mmx_slonczewski sl;  // jz = 0: off
+  bool relax_mode;     // stepping inside mmx_relax: the local kernels drop the precession term
   bool has_elastic;
   mmx_elastic el;
   bool use_demag;

@@ -115,3 +115,44 @@ def test_argument_errors_of_the_new_setters():
     with pytest.raises(mmx.MmxError):
         g.set_slonczewski(jz=1e11, mp=(0, 0, 1), **kw)          # Lambda < 1
     g.destroy()
+
+
+def test_relax_driver_matches_the_oracle_and_leaves_time_alone():
+    """mmx_relax (reading S39): damping-only torque, adaptive DP45 to a torque threshold.  Macrospin closed form on the
+    CUDA path (azimuth frozen, m_z = tanh), then a c2 film: the library and the oracle start from the same seeded state,
+    both stop below the threshold, the relaxed states agree (same minimum: |dm| small), the energy went down, the
+    simulation time did not move and ordinary stepping afterwards has its precession back."""
+    GAMMA = 1.7595e11
+    spec = wl.make("c1", (4, 1, 1))
+    spec.demag = False
+    spec.mat["alpha"][:] = 0.3
+    spec.mat["A"][:] = 0.0
+    spec.bext = (0.0, 0.0, 0.7)
+    m0 = np.array([0.48, 0.36, 0.8])
+    spec.m = [np.tile(m0.reshape(3, 1, 1, 1), (1, 1, 1, 4)).astype(np.float32)]
+    g = mmx.World.from_spec(spec)
+    st = g.relax(torque_stop=1e-4 * GAMMA, tol=1e-7)
+    m = g.get_state(mmx.F_M0)[:, 0, 0, 0].astype(np.float64)
+    assert st["accepted"] > 0 and g.get_time() == 0.0
+    assert abs(np.arctan2(m[1], m[0]) - np.arctan2(0.36, 0.48)) < 2e-6      # no precession
+    assert 1 - m[2] < 1e-6                                                  # relaxed along the field
+    g.destroy()
+
+    spec = wl.make("c2", (32, 32, 1))
+    g, o = pair(spec)
+    E0 = g.energy(mmx.T_ALL)
+    stop = 2e-3 * GAMMA
+    sg = g.relax(torque_stop=stop)
+    so = o.relax(stop)
+    assert sg["max_torque"] < stop and sg["rejected"] >= 0 and g.get_time() == 0.0
+    assert abs(sg["accepted"] - so["accepted"]) <= 2
+    assert max_dm(g.get_state(mmx.F_M0), o.m[0]) < 5e-4                      # same relaxed state (S21/S39: unpinned path)
+    assert g.energy(mmx.T_ALL) < E0
+    assert abs(g.energy(mmx.T_ALL) - o.energy(oc.T_ALL)) < 1e-4 * abs(o.energy(oc.T_ALL))
+    # precession is back: one fixed DP45 step equals the oracle's ordinary step from the relaxed state
+    o.m = [g.get_state(mmx.F_M0).astype(np.float64)]
+    o._k1 = None
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=2e-14, nsteps=5)
+    o.step_dp45_fixed(2e-14, 5)
+    assert max_dm(g.get_state(mmx.F_M0), o.m[0]) < 1e-5
+    g.destroy()
