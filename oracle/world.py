@@ -82,7 +82,10 @@ class World:
         """dict term-bit -> B_term for sublattice s (tesla)."""
         m = self.m if m is None else m
         p = self.p[s]
-        o = 1 - s if self.S == 2 else s
+        # partner sublattices: the inter-sublattice terms of Eq.3 / Eq.4 act between s and every other sublattice
+        # (two of them: the paper's s'; P:L120 "adding a third sublattice with the same interaction terms as the
+        # first two" -- reading S38: the terms are summed over both partners)
+        others = [t for t in range(self.S) if t != s]
         out = {}
         if terms & T_EXCH:
             out[T_EXCH] = fl.pair_laplacian(m[s], p["Ms"], p["A"], self.reg, self.cpl["scale_A11"],
@@ -100,26 +103,37 @@ class World:
             out[T_ZEEMAN] = fl.zeeman(m[s], p["Ms"], self.bext)
         if (terms & T_DEMAG) and self.use_demag:
             out[T_DEMAG] = self.demag_field(m) if b_demag is None else b_demag
-        if self.S == 2:
+        if self.S >= 2:
             if terms & T_A12:
                 A12 = np.full_like(p["Ms"], self.cpl["A12"])
-                out[T_A12] = fl.pair_laplacian(m[o], p["Ms"], A12, self.reg, self.cpl["scale_A12"],
-                                               self.cell, self.pbc, 1.0)
+                out[T_A12] = sum(fl.pair_laplacian(m[o], p["Ms"], A12, self.reg, self.cpl["scale_A12"],
+                                                   self.cell, self.pbc, 1.0) for o in others)
             if terms & T_A0:
-                out[T_A0] = fl.homogeneous_exchange(m[o], p["Ms"], self.cpl["A0"], self.cpl["latcon"])
+                out[T_A0] = sum(fl.homogeneous_exchange(m[o], p["Ms"], self.cpl["A0"], self.cpl["latcon"])
+                                for o in others)
             if terms & T_DMI_INTER:
                 Di = np.full_like(p["Ms"], self.cpl["D_inter"])
-                out[T_DMI_INTER] = fl.dmi_interfacial(m[o], p["Ms"], Di, self.cell, self.pbc)
+                out[T_DMI_INTER] = sum(fl.dmi_interfacial(m[o], p["Ms"], Di, self.cell, self.pbc) for o in others)
                 q12 = self.cpl.get("dmi_q12")
                 if q12 is not None and np.any(np.asarray(q12)):
                     # Eq.4 with s != s' ("a third DMI tensor is used to describe the intersublattice
                     # interaction", D^(s,s') = D^(s',s)): eps = sum_i q12_i . (m x d_i m' + m' x d_i m), whose
                     # variation gives B^(s) = (2/Ms^(s)) sum_i q12_i x d_i m^(s') -- the intra-sublattice
                     # expression with the partner's magnetisation (reading S33 for the tensor <-> q_i mapping)
-                    out[T_DMI_INTER] = out[T_DMI_INTER] + fl.dmi_tensor(m[o], p["Ms"], np.asarray(q12, float),
-                                                                        self.cell, self.pbc)
+                    for o in others:
+                        out[T_DMI_INTER] = out[T_DMI_INTER] + fl.dmi_tensor(m[o], p["Ms"], np.asarray(q12, float),
+                                                                            self.cell, self.pbc)
             if terms & T_DMI_HOMO:
-                out[T_DMI_HOMO] = fl.dmi_homogeneous(m[o], p["Ms"], self.cpl.get("d_homo", (0.0, 0.0, 0.0)), s)
+                # Eq.6 between the pairs (first, second) of reading S32: (0,1) for two sublattices, the cyclic
+                # pairs (0,1), (1,2), (2,0) for three (reading S38); s is the first spin of the pair (s, s+1)
+                # and the second spin of the pair (s-1, s)
+                d = self.cpl.get("d_homo", (0.0, 0.0, 0.0))
+                B = np.zeros_like(m[s])
+                if self.S == 3 or s == 0:
+                    B = B + fl.dmi_homogeneous(m[(s + 1) % self.S], p["Ms"], d, 0)
+                if self.S == 3 or s == 1:
+                    B = B + fl.dmi_homogeneous(m[(s - 1) % self.S], p["Ms"], d, 1)
+                out[T_DMI_HOMO] = B
         if (terms & T_MEL) and self.elastic is not None:
             u = self.u if u is None else u
             out[T_MEL] = fl.magnetoelastic_field(m[s], p["Ms"], p["B1"], p["B2"], self.strain(u))

@@ -322,3 +322,89 @@ def test_P22b_inter_sublattice_dmi_tensor_is_the_gradient_of_eq4():
         a = World(spec2).field_terms(s, terms=T_DMI_INTER)[T_DMI_INTER]
         b = World(spec3).field_terms(s, terms=T_DMI_INTER)[T_DMI_INTER]
         np.testing.assert_allclose(a, b, atol=1e-12 * np.abs(b).max())
+
+
+def _three_sublattice_spec(grid, pbc, seed):
+    rng = np.random.default_rng(seed)
+    spec = wl.make("c3", grid)
+    spec.S, spec.pbc, spec.regions, spec.demag, spec.J = 3, pbc, None, False, (0.0, 0.0, 0.0)
+    spec.cell = (2e-9, 2.5e-9, 1.5e-9)
+    spec.mat = wl.make_mat(3, Ms=np.array([[4e5], [7e5], [5e5]]), A=1e-11, alpha=0.1)
+    spec.coupling = wl.default_coupling(A0=-2.5e-11, A12=-1.5e-11, latcon=0.35e-9, D_inter=0.0,
+                                        d_homo=(2e5, -1e5, 1e6))
+    spec.m = [wl.random_unit(rng, grid) for _ in range(3)]
+    return spec
+
+
+def test_P25_three_sublattices_fields_are_the_gradient_of_the_pair_energies():
+    """P:L120 ("adding a third sublattice with the same interaction terms as the first two"; reading S38).  The
+    inter-sublattice energies are written out pair by pair, independently of the oracle's field code,
+        E = V sum_cells [ -(4 A0/a^2) sum_{s<s'} m_s.m_s'  -  A12 sum_{s<s'} m_s . lap m_s'  +  d . sum_cyc m_s x m_{s+1} ]
+    (periodic grid, 7-point Laplacian) and differentiated numerically; World.field_terms for each of the three
+    sublattices must be the gradient.  Pins the sums over both partners, the factor of each term and the cyclic
+    order of Eq.6 for three sublattices."""
+    grid = (5, 4, 3)
+    spec = _three_sublattice_spec(grid, (1, 1, 1), 44)
+    w = World(spec)
+    c = w.cpl
+    V = w.V
+
+    def lap(a):
+        out = np.zeros_like(a)
+        for ax, h in ((3, spec.cell[0]), (2, spec.cell[1]), (1, spec.cell[2])):
+            out += (np.roll(a, 1, axis=ax) + np.roll(a, -1, axis=ax) - 2 * a) / h ** 2
+        return out
+
+    def energy(m):
+        E = 0.0
+        for s in range(3):
+            for t in range(s + 1, 3):
+                E += -(4 * c["A0"] / c["latcon"] ** 2) * (m[s] * m[t]).sum() - c["A12"] * (m[s] * lap(m[t])).sum()
+            E += (np.asarray(c["d_homo"]).reshape(3, 1, 1, 1) * np.cross(m[s], m[(s + 1) % 3], axis=0)).sum()
+        return V * E
+
+    bits = T_A0 | T_A12 | T_DMI_HOMO
+    B = [w.heff(s, terms=bits) for s in range(3)]
+    scale = max(np.abs(b).max() for b in B)
+    rng = np.random.default_rng(5)
+    for _ in range(18):
+        s, comp = int(rng.integers(0, 3)), int(rng.integers(0, 3))
+        iz, iy, ix = (int(rng.integers(0, k)) for k in (grid[2], grid[1], grid[0]))
+        m0 = w.m[s][comp, iz, iy, ix]
+        E = []
+        for sgn in (+1, -1):
+            w.m[s][comp, iz, iy, ix] = m0 + sgn * 1e-4
+            E.append(energy(w.m))
+        w.m[s][comp, iz, iy, ix] = m0
+        want = -(E[0] - E[1]) / 2e-4 / (w.p[s]["Ms"][iz, iy, ix] * V)
+        assert abs(B[s][comp, iz, iy, ix] - want) < 1e-7 * scale, (s, comp)
+    assert abs(w.energy(bits) - energy(w.m)) < 1e-9 * abs(energy(w.m))
+
+
+def test_P25_the_120_degree_state_closed_forms():
+    """Three sublattices at 120 degrees in the plane, uniform: with the homogeneous exchange A0 < 0 alone every
+    sublattice feels B = -(4 A0/(Ms a^2)) m_s -- parallel to m_s, so the torque vanishes exactly -- and the energy is
+    (3/2)(4 A0/a^2) V per cell; a DMI vector d z^ adds +-(3 sqrt(3)/2) d V per cell, the sign being the chirality
+    (the sense in which sublattices 0 -> 1 -> 2 go round), which pins the cyclic order of Eq.6 for S = 3."""
+    grid = (4, 3, 1)
+    n = grid[0] * grid[1] * grid[2]
+    spec = _three_sublattice_spec(grid, (0, 0, 0), 1)
+    spec.coupling.update(A12=0.0, d_homo=(0.0, 0.0, 0.0))
+    spec.mat["A"][:] = 0.0
+    ang = lambda k, chi: np.array([np.cos(chi * 2 * np.pi * k / 3 + 0.3), np.sin(chi * 2 * np.pi * k / 3 + 0.3), 0.0])
+    for chi in (+1, -1):
+        s2 = spec.copy()
+        s2.m = [np.tile(ang(k, chi).reshape(3, 1, 1, 1), (1, grid[2], grid[1], grid[0])).astype(np.float32) for k in range(3)]
+        w = World(s2)
+        w.m = [np.tile(ang(k, chi).reshape(3, 1, 1, 1), (1, grid[2], grid[1], grid[0])) for k in range(3)]
+        pref = 4 * w.cpl["A0"] / w.cpl["latcon"] ** 2
+        for s in range(3):
+            B = w.heff(s, terms=T_A0)
+            np.testing.assert_allclose(B, -(pref / w.p[s]["Ms"])[None] * w.m[s], rtol=1e-12)
+            assert np.abs(w.torque(s, terms=T_A0)).max() < 1e-6 * GAMMA_ * abs(pref) / 4e5
+        np.testing.assert_allclose(w.energy(T_A0), 1.5 * pref * w.V * n, rtol=1e-12)
+        w.cpl["d_homo"] = (0.0, 0.0, 1.0e6)
+        np.testing.assert_allclose(w.energy(T_DMI_HOMO), chi * 1.5 * np.sqrt(3.0) * 1.0e6 * w.V * n, rtol=1e-12)
+
+
+GAMMA_ = 1.7595e11

@@ -37,7 +37,7 @@ class WorldSpec:
     grid: tuple            # (Nx, Ny, Nz)
     cell: tuple            # (dx, dy, dz) in metres
     pbc: tuple = (0, 0, 0)  # periodic image repetitions per axis, 0 = open
-    S: int = 1              # number of sublattices (1 or 2)
+    S: int = 1              # number of sublattices (1, 2 or 3)
     regions: np.ndarray | None = None   # uint16 [Nz,Ny,Nx]; None = one region
     mat: dict = field(default_factory=dict)       # name -> float64 [S,R] or [S,R,3]
     coupling: dict = field(default_factory=dict)  # A0, A12, latcon, D_inter, scale_A11, scale_A12
