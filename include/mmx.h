@@ -64,7 +64,7 @@ enum {
 };
 
 /* state fields for mmx_set_state / mmx_get_state */
-enum { MMX_F_M0 = 0, MMX_F_M1 = 1, MMX_F_U = 2, MMX_F_V = 3 };
+enum { MMX_F_M0 = 0, MMX_F_M1 = 1, MMX_F_U = 2, MMX_F_V = 3, MMX_F_M2 = 4 /* third sublattice */ };
 
 /* Runge-Kutta methods (Table 2; RK4 = classical, not in the table) */
 enum {
@@ -156,7 +156,9 @@ const char* mmx_version(void);
  *   cellsize[3] = (dx, dy, dz) in m
  *   pbc[3]      = number of periodic image repetitions per axis used by the demag kernel;
  *                 0 = open axis.  A periodic axis must have a power-of-two size.
- *   n_sublattices = 1 (ferromagnet) or 2 (antiferro-/ferrimagnet)
+ *   n_sublattices = 1 (ferromagnet), 2 (antiferro-/ferrimagnet) or 3 (non-collinear antiferromagnet: "a third
+ *   sublattice with the same interaction terms as the first two": the inter-sublattice terms are summed over both partners,
+ *   Eq.6 runs over the cyclic pairs (0,1), (1,2), (2,0); reading S38)
  *   cuda_stream = cudaStream_t (as void*) on which all work is enqueued.  NULL: the library
  *                 creates its own blocking stream (the legacy default stream cannot be captured
  *                 into the step graph); the runtime orders that stream against the legacy default

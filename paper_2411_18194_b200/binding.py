@@ -18,7 +18,8 @@ HOST, DEVICE = 0, 1
 T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0, T_DMI_INTER, T_MEL, T_DMI_HOMO = (
     1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1024)
 T_ALL = 2047
-F_M0, F_M1, F_U, F_V = 0, 1, 2, 3
+F_M0, F_M1, F_U, F_V, F_M2 = 0, 1, 2, 3, 4
+F_M = (F_M0, F_M1, F_M2)   # state field id of sublattice s
 DMI_INTER = -1
 RK4, DP45, HEUN12, BS23, CK45, RKF45 = 0, 1, 2, 3, 4, 5
 FACES = {"x-": 0, "x+": 1, "y-": 2, "y+": 3, "z-": 4, "z+": 5}
@@ -405,7 +406,7 @@ class World:
         if spec.elastic is not None:
             w.set_elastic(spec.elastic)
         for s in range(spec.S):
-            w.set_state(F_M0 + s, np.ascontiguousarray(spec.m[s], dtype=np.float32))
+            w.set_state(F_M[s], np.ascontiguousarray(spec.m[s], dtype=np.float32))
         if spec.elastic is not None:
             w.set_state(F_U, np.ascontiguousarray(spec.u, dtype=np.float32))
             w.set_state(F_V, np.ascontiguousarray(spec.v, dtype=np.float32))

@@ -227,7 +227,7 @@ unsigned active_terms(const mmx_world* w) {
   unsigned t = MMX_T_ALL;
   if (!(w->use_demag && w->dm.ready)) t &= ~MMX_T_DEMAG;
   if (!w->has_elastic) t &= ~MMX_T_MEL;
-  if (w->S != 2) t &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER | MMX_T_DMI_HOMO);
+  if (w->S < 2) t &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER | MMX_T_DMI_HOMO);
   return t;
 }
 
@@ -252,10 +252,10 @@ void fill_local(const mmx_world* w, LocalArgs& a, unsigned terms) {
   for (int k = 0; k < 3; ++k) a.dhomo[k] = (float)w->cpl.d_homo[k];
   a.has_dmiq = w->has_dmiq ? 1 : 0;
   a.has_dmiq12 = 0;
-  for (int s = 0; s < 3; ++s)
+  for (int s = 0; s < 4; ++s)
     for (int k = 0; k < 9; ++k) {
       a.dmiq[s][k / 3][k % 3] = (float)w->dmiq[s][k];
-      if (s == 2 && w->dmiq[s][k] != 0.0) a.has_dmiq12 = 1;
+      if (s == 3 && w->dmiq[s][k] != 0.0) a.has_dmiq12 = 1;
     }
   a.has_sl = w->sl.jz != 0.0 ? 1 : 0;
   {
@@ -561,7 +561,7 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
                      void* cuda_stream, mmx_world** out) {
   if (!grid || !cellsize || !pbc || !out) return mmx_fail(MMX_EINVAL, "NULL argument");
   *out = nullptr;
-  if (n_sublattices < 1 || n_sublattices > 2) return mmx_fail(MMX_EINVAL, "n_sublattices must be 1 or 2");
+  if (n_sublattices < 1 || n_sublattices > 3) return mmx_fail(MMX_EINVAL, "n_sublattices must be 1, 2 or 3");
   for (int a = 0; a < 3; ++a) {
     if (grid[a] < 1) return mmx_fail(MMX_EINVAL, "grid[%d] = %d", a, grid[a]);
     if (!(cellsize[a] > 0)) return mmx_fail(MMX_EINVAL, "cellsize[%d] must be > 0", a);
@@ -589,7 +589,7 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
     else { cudaGetLastError(); w->stream = nullptr; }
   }
   w->has_dmiq = false;
-  for (int s = 0; s < 3; ++s)
+  for (int s = 0; s < 4; ++s)
     for (int k = 0; k < 9; ++k) w->dmiq[s][k] = 0.0;
   memset(&w->sl, 0, sizeof(w->sl));
   w->relax_mode = false;
@@ -729,14 +729,14 @@ int mmx_set_current(mmx_world* w, const double J[3]) {
 int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]) {
   if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
   if (sublattice == MMX_DMI_INTER) {
-    if (w->S != 2) return mmx_fail(MMX_EINVAL, "the inter-sublattice DMI tensor needs two sublattices");
-    sublattice = 2;
+    if (w->S < 2) return mmx_fail(MMX_EINVAL, "the inter-sublattice DMI tensor needs two or three sublattices");
+    sublattice = 3;
   } else if (sublattice < 0 || sublattice >= w->S) {
     return mmx_fail(MMX_EINVAL, "sublattice %d out of range", sublattice);
   }
   for (int k = 0; k < 9; ++k) w->dmiq[sublattice][k] = q ? q[k] : 0.0;
   w->has_dmiq = false;
-  for (int s = 0; s < 3; ++s)
+  for (int s = 0; s < 4; ++s)
     for (int k = 0; k < 9; ++k) w->has_dmiq = w->has_dmiq || w->dmiq[s][k] != 0.0;
   w->k1_valid = false;
   w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
@@ -791,6 +791,9 @@ static int field_vec(mmx_world* w, int field, int* vec) {
     case MMX_F_M1:
       if (w->S < 2) return mmx_fail(MMX_EINVAL, "world has one sublattice");
       *vec = 1; return MMX_OK;
+    case MMX_F_M2:
+      if (w->S < 3) return mmx_fail(MMX_EINVAL, "world has fewer than three sublattices");
+      *vec = 2; return MMX_OK;
     case MMX_F_U:
     case MMX_F_V:
       if (!w->has_elastic) return mmx_fail(MMX_ESTATE, "elastic fields need mmx_set_elastic first");
@@ -918,7 +921,7 @@ int mmx_eval_heff(mmx_world* w, int sublattice, unsigned term_mask, float* out, 
   if (int rc = prepare(w)) return rc;
   unsigned terms = term_mask;
   if (!w->has_elastic) terms &= ~MMX_T_MEL;
-  if (w->S != 2) terms &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER | MMX_T_DMI_HOMO);
+  if (w->S < 2) terms &= ~(MMX_T_A12 | MMX_T_A0 | MMX_T_DMI_INTER | MMX_T_DMI_HOMO);
   if (int rc = eval_prereq(w, terms)) return rc;
   LocalArgs la;
   fill_local(w, la, terms);

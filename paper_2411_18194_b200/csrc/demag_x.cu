@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
 
 bool mmx_x_warp_ok(const mmx_world* w) {
   const DemagPlan& d = w->dm;
-  if (d.px != XP || (d.nx & 3) || d.nx > XH || w->nreg != 1) return false;
+  if (d.px != XP || (d.nx & 3) || d.nx > XH || w->nreg != 1 || w->S > 2) return false;
   for (int s = 0; s < w->S; ++s)
     if (!(w->mats[(size_t)s * w->nreg].Ms > 0)) return false;
   return true;

@@ -114,11 +114,11 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
       if (a.heff_out || a.tau_out) {
         if (s != a.heff_s) continue;
       }
-      const int o = S == 2 ? 1 - s : s;
+      // partner sublattices o = (s + t) mod S, t = 1 .. S - 1: the inter-sublattice terms act between s and every
+      // other sublattice (reading S38)
       const float* P = a.mat + ((size_t)s * a.nreg + rc) * MMX_MATW;
       const float Ms = P[MP_MS], iMs = P[MP_INVMS];
       const float* ms_ = yin + (size_t)s * 3 * N;
-      const float* mo_ = yin + (size_t)o * 3 * N;
       V3 B = v3(0.f, 0.f, 0.f);
       V3 dm = v3(0.f, 0.f, 0.f);  // (u.grad) m for Zhang-Li
       V3 tau = v3(0.f, 0.f, 0.f);
@@ -150,9 +150,11 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
                 const V3 qv = v3(a.dmiq[s][axis][0], a.dmiq[s][axis][1], a.dmiq[s][axis][2]);
                 B = fma3(iMs * a.inv_h[axis] * d, cross(qv, mn), B);
               }
-              if (S == 2) {
-                if (a.terms & (MMX_T_A12 | MMX_T_DMI_INTER)) {
-                  const V3 on = ld3(mo_, N, (size_t)ni[q]);
+              if (S >= 2 && (a.terms & (MMX_T_A12 | MMX_T_DMI_INTER))) {
+#pragma unroll
+                for (int t = 1; t < S; ++t) {
+                  const int o = (s + t) % S;
+                  const V3 on = ld3(yin + (size_t)o * 3 * N, N, (size_t)ni[q]);
                   if (a.terms & MMX_T_A12) {
                     const float w12 = a.A12 * (same ? 1.f : a.scaleA12) * iMs * a.inv_h2[axis];
                     B = fma3(w12, on - mc[o], B);
@@ -164,7 +166,7 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
                   }
                   if (a.has_dmiq12 && (a.terms & MMX_T_DMI_INTER)) {
                     // inter-sublattice tensor of Eq.4: B_c += d /(Ms_c h_i) q12_i x m'_n
-                    const V3 qv = v3(a.dmiq[2][axis][0], a.dmiq[2][axis][1], a.dmiq[2][axis][2]);
+                    const V3 qv = v3(a.dmiq[3][axis][0], a.dmiq[3][axis][1], a.dmiq[3][axis][2]);
                     B = fma3(iMs * a.inv_h[axis] * d, cross(qv, on), B);
                   }
                 }
@@ -177,11 +179,16 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
             dm = fma3(wu, mn, dm);
           }
         }
-        if (S == 2 && (a.terms & MMX_T_A0)) B = fma3(a.a0pref * iMs, mc[o], B);
-        if (S == 2 && (a.terms & MMX_T_DMI_HOMO)) {
-          // Eq.6: eps = d . (m1 x m2)  =>  B1 = (d x m2)/Ms1,  B2 = (m1 x d)/Ms2
+        if (S >= 2 && (a.terms & MMX_T_A0)) {
+#pragma unroll
+          for (int t = 1; t < S; ++t) B = fma3(a.a0pref * iMs, mc[(s + t) % S], B);
+        }
+        if (S >= 2 && (a.terms & MMX_T_DMI_HOMO)) {
+          // Eq.6: eps = d . (m_a x m_b)  =>  B_a = (d x m_b)/Ms_a,  B_b = (m_a x d)/Ms_b; pairs (a, b) = (0, 1) for two
+          // sublattices, the cyclic pairs (0,1), (1,2), (2,0) for three (readings S32, S38)
           const V3 dv = v3(a.dhomo[0], a.dhomo[1], a.dhomo[2]);
-          B = fma3(iMs, s == 0 ? cross(dv, mc[o]) : cross(mc[o], dv), B);
+          if (S == 3 || s == 0) B = fma3(iMs, cross(dv, mc[(s + 1) % S]), B);
+          if (S == 3 || s == 1) B = fma3(iMs, cross(mc[(s + S - 1) % S], dv), B);
         }
         if (a.terms & MMX_T_ANIS_U) {
           const V3 u = v3(P[MP_UX], P[MP_UY], P[MP_UZ]);
@@ -970,6 +977,7 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   // (the general DMI tensors and the Slonczewski torque live in the general kernel k_local only)
   bool uniform = !reg && (w->grid[0] % 4) == 0 && !a.has_dmiq && !a.has_sl;
   for (int s = 0; s < w->S && uniform; ++s) uniform = w->mats[(size_t)s * w->nreg].Ms > 0;
+  if (w->S > 2) uniform = false;  // (three sublattices: general kernel)
   const bool open_all = !a.per[0] && !a.per[1] && !a.per[2];
   if (uniform && w->S == 1 && open_all) {
     // TMA halo tiles (k_local_t)
@@ -1018,9 +1026,12 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   } else if (w->S == 1) {
     if (reg) k_local<1, true><<<blocks, 256, 0, w->stream>>>(a);
     else k_local<1, false><<<blocks, 256, 0, w->stream>>>(a);
-  } else {
+  } else if (w->S == 2) {
     if (reg) k_local<2, true><<<blocks, 256, 0, w->stream>>>(a);
     else k_local<2, false><<<blocks, 256, 0, w->stream>>>(a);
+  } else {
+    if (reg) k_local<3, true><<<blocks, 256, 0, w->stream>>>(a);
+    else k_local<3, false><<<blocks, 256, 0, w->stream>>>(a);
   }
   w->launches++;
   MMX_CUDA(cudaGetLastError());

@@ -63,7 +63,7 @@ struct LocalArgs {
   const float* mat;      // [S][nreg][MMX_MATW]
   float scaleA11, scaleA12, A12, a0pref, Dinter;
   float dhomo[3];        // DMI vector of Eq.6, J/m^3
-  float dmiq[3][3][3];   // general DMI tensor of Eq.4 as per-axis vectors q_i: sublattice 0, 1, inter-sublattice; J/m^2
+  float dmiq[4][3][3];   // general DMI tensor of Eq.4 as per-axis vectors q_i: sublattice 0, 1, 2, inter-sublattice; J/m^2
   int has_dmiq;          // any tensor set (routes the world to the general kernel)
   int has_dmiq12;        // the inter-sublattice one
   // Slonczewski torque (reading S37)
@@ -168,7 +168,7 @@ struct mmx_world {
   bool mat_dirty;
   mmx_coupling cpl;
   double bext[3], J[3];
-  double dmiq[3][9];   // general DMI tensors (mmx_set_dmi_tensor): sublattice 0, 1, inter-sublattice; zero = none
+  double dmiq[4][9];   // general DMI tensors (mmx_set_dmi_tensor): sublattice 0, 1, 2, inter-sublattice; zero = none
   bool has_dmiq;
   mmx_slonczewski sl;  // jz = 0: off
   bool relax_mode;     // stepping inside mmx_relax: the local kernels drop the precession term

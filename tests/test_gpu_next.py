@@ -156,3 +156,71 @@ def test_relax_driver_matches_the_oracle_and_leaves_time_alone():
     o.step_dp45_fixed(2e-14, 5)
     assert max_dm(g.get_state(mmx.F_M0), o.m[0]) < 1e-5
     g.destroy()
+
+
+def _three_sublattice_spec(grid, pbc, seed, regions=True):
+    rng = np.random.default_rng(seed)
+    spec = _rich_spec("c3", grid, seed=seed)          # grains, anisotropy axes, current: the c3 recipe ...
+    R = spec.n_regions
+    spec.S, spec.pbc = 3, pbc
+    for k, tab in list(spec.mat.items()):              # ... with a third sublattice appended to every material table
+        spec.mat[k] = np.concatenate([tab, tab[:1]], axis=0)
+    spec.mat["Ms"][2] = 5.0e5
+    spec.mat["D"][2] = 0.7e-3
+    spec.mat["Ku1"][2] = 8e4
+    if not regions:
+        spec.regions = None
+        for k, tab in list(spec.mat.items()):
+            spec.mat[k] = tab[:, :1].copy()
+    spec.coupling.update(A0=-2.5e-11, A12=-1.5e-12, D_inter=0.4e-3, d_homo=(2e5, -1e5, 1e6))
+    spec.m = [wl.random_unit(rng, grid) for _ in range(3)]
+    return spec
+
+
+@pytest.mark.parametrize("grid,pbc,regions", [((48, 24, 1), (0, 0, 0), True), ((32, 16, 1), (2, 2, 0), False),
+                                              ((20, 12, 4), (0, 0, 0), True)])
+def test_three_sublattices(grid, pbc, regions):
+    """P:L120, reading S38: a non-collinear antiferromagnet with three exchange-coupled sublattices (Fig.3's kind of
+    world: grains, reduced inter-grain exchange, interfacial + homogeneous DMI).  Every inter-sublattice term, the demag
+    field of M = sum_s Ms m_s, the total field, torque and energy of each sublattice, and a 20-step trajectory."""
+    spec = _three_sublattice_spec(grid, pbc, 61, regions)
+    spec.coupling["dmi_q12"] = 1e-3 * np.random.default_rng(2).standard_normal((3, 3))
+    g, o = pair(spec)
+    for s in range(3):
+        ref = o.field_terms(s)
+        for bit in (mmx.T_A12, mmx.T_A0, mmx.T_DMI_INTER, mmx.T_DMI_HOMO, mmx.T_DEMAG, mmx.T_EXCH, mmx.T_DMI):
+            assert field_err(g.eval_heff(s, bit), ref[bit]) < FIELD_TOL, (s, bit)
+        assert field_err(g.eval_heff(s, mmx.T_ALL), o.heff(s)) < FIELD_TOL, s
+        assert field_err(g.eval_torque(s), o.torque(s)) < FIELD_TOL, s
+    for bit in (mmx.T_A0, mmx.T_A12, mmx.T_DMI_HOMO, mmx.T_ALL):
+        Eg, Eo = g.energy(bit), o.energy(bit)
+        assert abs(Eg - Eo) < 2e-5 * abs(Eo), bit
+    dt = 2e-15
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=20)
+    o.step_dp45_fixed(dt, 20)
+    for s in range(3):
+        assert max_dm(g.get_state(mmx.F_M[s]), o.m[s]) <= TRAJ_TOL
+    g.destroy()
+
+
+def test_the_120_degree_state_is_an_equilibrium_of_the_cuda_path():
+    """P25's closed form end to end: three sublattices at 120 degrees under the homogeneous exchange alone: zero torque
+    (to fp32 rounding of a 300 T exchange field), B_s = -(4 A0/(Ms a^2)) m_s."""
+    grid = (8, 4, 1)
+    spec = _three_sublattice_spec(grid, (0, 0, 0), 3, regions=False)
+    spec.demag, spec.J = False, (0.0, 0.0, 0.0)
+    spec.coupling.update(A12=0.0, D_inter=0.0, d_homo=(0.0, 0.0, 0.0))
+    for k in ("A", "D", "Ku1", "Kc1"):
+        spec.mat[k][:] = 0.0
+    spec.bext = (0.0, 0.0, 0.0)
+    spec.m = [np.tile(np.array([np.cos(2 * np.pi * k / 3 + 0.3), np.sin(2 * np.pi * k / 3 + 0.3), 0.0]).reshape(3, 1, 1, 1),
+                      (1, 1, grid[1], grid[0])).astype(np.float32) for k in range(3)]
+    g = mmx.World.from_spec(spec)
+    pref = 4 * spec.coupling["A0"] / spec.coupling["latcon"] ** 2
+    for s in range(3):
+        B = g.eval_heff(s, mmx.T_ALL & ~mmx.T_DEMAG).astype(np.float64)
+        want = -(pref / spec.mat["Ms"][s, 0]) * spec.m[s].astype(np.float64)
+        assert np.abs(B - want).max() < 1e-6 * np.abs(want).max()
+        tau = g.eval_torque(s).astype(np.float64)
+        assert np.abs(tau).max() < 1e-6 * 1.7595e11 * np.abs(want).max()
+    g.destroy()
