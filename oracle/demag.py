@@ -85,3 +85,30 @@ def demag_fft(M, spectrum, grid, pbc):
         b = sfft.irfftn(acc, s=(P[2], P[1], P[0]), axes=(0, 1, 2), workers=-1)
         B[i] = -MU0 * b[:nz, :ny, :nx]
     return B
+
+
+def stray_field_at_height(M, grid, cell, height, cutoff_cells=32.0):
+    """Field of the magnet in a probe layer above it ("we calculate the out-of-plane component of the magnet's
+    stray field 60 nm above the film's surface"; reading S40: the probe layer has the magnet's in-plane grid and cell
+    size, its cells are centred `height` above the top surface, and the value is the average over a probe cell, like
+    every field of the method).  The definition, term by term:
+        B_i(x, y) = -mu0 sum_{x', y', k} sum_j N_ij(x - x', y - y', Dz_k) M_j(x', y', k),
+        Dz_k = (Nz - k - 1/2) dz + height           (centre of source layer k to centre of the probe layer),
+    N the cell-to-cell Newell tensor of oracle/newell.py at a z offset that is not a multiple of dz.  Open boundaries.
+    M float64 [3, Nz, Ny, Nx] in A/m; returns B [3, Ny, Nx] in tesla."""
+    nx, ny, nz = grid
+    iy, ix = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    B = np.zeros((3, ny, nx))
+    for k in range(nz):
+        dzk = (nz - k - 0.5) * cell[2] + height
+        quad = {c: nw.newell_octant(c, (nx, ny, 1), cell, cutoff_cells, shift=(0.0, 0.0, dzk))[0] for c in nw.COMPS}
+        for ty in range(ny):
+            for tx in range(nx):
+                dx, dy = tx - ix, ty - iy
+                for c in nw.COMPS:
+                    par = nw.PARITY[c]
+                    Kc = np.where(dx < 0, par[0], 1.0) * np.where(dy < 0, par[1], 1.0) * quad[c][np.abs(dy), np.abs(dx)]
+                    for (i, j), name in _PAIR.items():
+                        if name == c:
+                            B[i, ty, tx] += -MU0 * np.sum(Kc * M[j, k])
+    return B

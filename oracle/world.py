@@ -73,6 +73,11 @@ class World:
             self._spectrum = dm.kernel_spectrum(self.octant(), self.grid, self.pbc)
         return dm.demag_fft(M, self._spectrum, self.grid, self.pbc)
 
+    def stray_field(self, height, m=None):
+        """B [3, Ny, Nx] in a probe layer `height` above the top surface (reading S40), of M = sum_s Ms m_s."""
+        return dm.stray_field_at_height(self.magnetisation(self.m if m is None else m), self.grid, self.cell, height,
+                                        self.spec.cutoff_cells)
+
     # ------------------------------------------------------------------ fields
     def strain(self, u=None):
         u = self.u if u is None else u

@@ -157,3 +157,47 @@ def test_pbc_kernel_against_explicit_images():
     # difference = edge images that one window has and the other has not: O((cell/(R L))^3) each
     assert np.abs(Bp - Bo).max() < 2e-2 * np.abs(Bo).max()
     assert np.abs(Bp - Bo).max() > 0  # the windows do differ (definition, not identity)
+
+
+def test_P26_stray_field_above_the_magnet():
+    """P26 (pins oracle/demag.py::stray_field_at_height, reading S40).
+    (a) closed form: on the axis of a uniformly z-magnetised square slab (side a, thickness t) the surface-charge
+        picture gives B_z(z) = (mu0 Ms / 4 pi) [Omega(z - t/2) - Omega(z + t/2)], Omega(d) = 4 atan(a^2/(4 d sqrt(d^2 + a^2/2)))
+        the solid angle of the square seen from distance d; probe cells small against the height, so the cell average
+        equals the point value to O((cell/height)^2).
+    (b) far field: one magnetised cell seen from 40 cells above is a point dipole.
+    (c) tie to the validated in-magnet kernel (P4, P5): in a two-layer magnet the field that layer 0 alone creates in
+        layer 1 is the stray field of layer 0 at height dz/2 above its surface."""
+    from oracle import demag as dm
+    from oracle.constants import MU0
+    # (a)
+    n, h, t, Ms = 21, 2e-9, 3e-9, 8e5
+    M = np.zeros((3, 1, n, n)); M[2] = Ms
+    a = n * h
+    for height in (20e-9, 60e-9):
+        B = dm.stray_field_at_height(M, (n, n, 1), (h, h, t), height)
+        zc = t / 2 + height                                   # probe centre above the slab centre
+        om = lambda d: 4 * np.arctan(a * a / (4 * d * np.sqrt(d * d + a * a / 2)))
+        want = MU0 * Ms / (4 * np.pi) * (om(zc - t / 2) - om(zc + t / 2))
+        assert abs(B[2, n // 2, n // 2] - want) < 2e-3 * abs(want), (height, B[2, n // 2, n // 2], want)
+        assert abs(B[0, n // 2, n // 2]) < 1e-9 * abs(want) and abs(B[1, n // 2, n // 2]) < 1e-9 * abs(want)
+    # (b)
+    n, h = 9, 1e-9
+    M = np.zeros((3, 1, n, n)); mom = np.array([0.3, -0.5, 0.8]) * 1e6
+    M[:, 0, 4, 4] = mom
+    height = 40e-9
+    B = dm.stray_field_at_height(M, (n, n, 1), (h, h, h), height, cutoff_cells=8.0)
+    for (ty, tx) in ((4, 4), (0, 8), (7, 2)):
+        r = np.array([(tx - 4) * h, (ty - 4) * h, h / 2 + height])
+        rn = np.linalg.norm(r)
+        want = MU0 / (4 * np.pi) * h ** 3 * (3 * r * (mom @ r) / rn ** 5 - mom / rn ** 3)
+        np.testing.assert_allclose(B[:, ty, tx], want, rtol=2e-3, atol=1e-6 * np.abs(want).max())
+    # (c)
+    rng = np.random.default_rng(8)
+    grid, cell = (6, 5, 2), (2e-9, 3e-9, 1.5e-9)
+    M = rng.standard_normal((3, 2, 5, 6)) * 5e5
+    M0 = M.copy(); M0[:, 1] = 0.0
+    octant = nw.kernel_octant(grid, cell)
+    ref = dm.demag_direct(M0, octant, grid, (0, 0, 0))[:, 1]
+    got = dm.stray_field_at_height(M0[:, :1], (6, 5, 1), cell, cell[2] / 2)
+    np.testing.assert_allclose(got, ref, rtol=1e-10, atol=1e-12 * np.abs(ref).max())
