@@ -254,6 +254,14 @@ int mmx_elastic_energy(mmx_world* w, double* strain_energy, double* kinetic_ener
 /* max over cells and sublattices of |tau| (1/s). */
 int mmx_max_torque(mmx_world* w, double* out);
 
+/* Field of the magnet in a probe layer above it ("we calculate the out-of-plane component of the magnet's stray
+ * field 60 nm above the film's surface", Fig.3; reading S40): the probe layer has the magnet's in-plane grid and
+ * cell size, its cells are centred `height` metres above the top surface (height > -cellsize[2]/2), values are averages
+ * over a probe cell.  B_i = -mu0 sum N_ij(x - x', y - y', Dz_k) M_j over all cells of all layers, M = sum_s Ms m_s, N the
+ * Newell tensor at the real z offset Dz_k = (Nz - k - 1/2) dz + height.  Open boundaries only (MMX_EINVAL otherwise).
+ * out: fp32 [3][Ny][Nx] tesla, host or device.  A direct sum: meant for imaging a state, not for the time loop. */
+int mmx_stray_field(mmx_world* w, double height, float* out, int mem);
+
 /* ---- time stepping --------------------------------------------------------------------- */
 
 /* nsteps classical RK4 steps of size dt (BASELINE config 1 protocol). */

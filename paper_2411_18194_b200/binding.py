@@ -103,6 +103,7 @@ PROTOTYPES = {
     "mmx_max_torque": (C.c_int, [_W, _D3]),
     "mmx_step_rk4": (C.c_int, [_W, C.c_double, C.c_longlong]),
     "mmx_step_rk45": (C.c_int, [_W, C.POINTER(RkOpts), C.POINTER(RkStats)]),
+    "mmx_stray_field": (C.c_int, [_W, C.c_double, C.c_void_p, C.c_int]),
     "mmx_relax": (C.c_int, [_W, C.c_double, C.c_double, C.c_longlong, C.POINTER(RkStats)]),
     "mmx_get_err_history": (C.c_int, [_W, _D3, C.c_int, _I3]),
     "mmx_profile_enable": (C.c_int, [_W, C.c_int]),
@@ -338,6 +339,13 @@ class World:
         st = RkStats()
         _check(self.lib.mmx_step_rk45(self.h, C.byref(o), C.byref(st)))
         return {k: getattr(st, k) for k, _ in RkStats._fields_}
+
+    def stray_field(self, height):
+        """B [3, Ny, Nx] (tesla, fp32) in a probe layer `height` metres above the top surface."""
+        out = np.empty((3, self.grid[1], self.grid[0]), dtype=np.float32)
+        p, mem = _ptr_mem(out)
+        _check(self.lib.mmx_stray_field(self.h, float(height), p, mem))
+        return out
 
     def relax(self, torque_stop, tol=1e-5, max_attempts=0):
         st = RkStats()

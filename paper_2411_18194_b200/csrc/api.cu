@@ -1032,6 +1032,24 @@ int mmx_max_torque(mmx_world* w, double* out) {
   return MMX_OK;
 }
 
+int mmx_stray_field(mmx_world* w, double height, float* out, int mem) {
+  if (!w || !out) return mmx_fail(MMX_EINVAL, "NULL argument");
+  if (w->pbc[0] || w->pbc[1] || w->pbc[2]) return mmx_fail(MMX_EINVAL, "mmx_stray_field needs open boundaries");
+  if (!(height > -0.5 * w->cell[2])) return mmx_fail(MMX_EINVAL, "the probe layer must lie above the centre of the top layer");
+  if (int rc = prepare(w)) return rc;
+  const size_t cnt = (size_t)3 * w->grid[0] * w->grid[1];
+  float* dst = out;
+  float* tmp = nullptr;
+  if (mem == MMX_HOST) {
+    MMX_CUDA(cudaMalloc(&tmp, cnt * sizeof(float)));
+    dst = tmp;
+  }
+  int rc = mmx_stray_launch(w, height, 0.0, dst);
+  if (!rc && mem == MMX_HOST) rc = copy_out(w, tmp, out, MMX_HOST, cnt);
+  cudaFree(tmp);
+  return rc;
+}
+
 int mmx_step_rk4(mmx_world* w, double dt, long long nsteps) {
   if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
   if (!(dt > 0) || nsteps < 0) return mmx_fail(MMX_EINVAL, "dt must be > 0 and nsteps >= 0");

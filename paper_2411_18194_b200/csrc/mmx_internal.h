@@ -303,6 +303,9 @@ int mmx_combine_launch(mmx_world* w, const float* const y0[2], const float* cons
 int mmx_controller_launch(mmx_world* w, const MmxTableau& tab, int mode);
 int mmx_energy_launch(mmx_world* w, unsigned term_mask, const float* bdemag, double* host_out);
 
+// stray.cu
+int mmx_stray_launch(mmx_world* w, double height, double cutoff_cells, float* dev_out);
+
 // elastic.cu
 int mmx_strain_launch(mmx_world* w, const ElasticArgs& a);
 int mmx_elastic_launch(mmx_world* w, const ElasticArgs& a);

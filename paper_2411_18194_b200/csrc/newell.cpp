@@ -279,3 +279,16 @@ int mmx_kernel_spectrum(const int grid[3], const int pbc[3], const int P[3], int
   (void)grid; (void)pbc;
   return MMX_OK;
 }
+
+// N_comp(i dx, j dy, dz) on the non-negative quadrant of in-plane offsets at a fixed z offset dz (any real number, not
+// a multiple of the cell height): the cell-to-cell tensor between a source layer and a probe layer above the magnet
+// (mmx_stray_field).  out: [6][ny][nx].
+int mmx_newell_quadrant_at(int nx, int ny, const double cell[3], double dz, double cutoff_cells, std::vector<double>& out) {
+  if (cutoff_cells <= 0) cutoff_cells = 32.0;
+  const int n[3] = {nx, ny, 1};
+  const size_t cnt = (size_t)nx * ny;
+  out.assign(6 * cnt, 0.0);
+  const double shift[3] = {0.0, 0.0, dz};
+  for (int comp = 0; comp < 6; ++comp) add_octant(comp, n, cell, cutoff_cells, shift, out.data() + comp * cnt);
+  return MMX_OK;
+}

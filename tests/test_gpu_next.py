@@ -224,3 +224,42 @@ def test_the_120_degree_state_is_an_equilibrium_of_the_cuda_path():
         tau = g.eval_torque(s).astype(np.float64)
         assert np.abs(tau).max() < 1e-6 * 1.7595e11 * np.abs(want).max()
     g.destroy()
+
+
+@pytest.mark.parametrize("name,grid,height", [("c1", (40, 24, 1), 60e-9), ("c4", (20, 18, 3), 7e-9), ("three", (36, 20, 1), 60e-9)])
+def test_stray_field_above_the_magnet(name, grid, height):
+    """P:L84, Fig.3; reading S40: the field in a probe layer above the magnet against the oracle's term-by-term sum with the
+    z-shifted Newell tensor: one layer, several layers (each with its own z offset), and the Fig.3 kind of world (three
+    sublattices with different Ms and grains, M = sum_s Ms m_s; cell 1 x 1 x 30 nm, probe 60 nm above the surface)."""
+    if name == "three":
+        spec = _three_sublattice_spec(grid, (0, 0, 0), 71)
+        spec.cell = (1e-9, 1e-9, 30e-9)
+    else:
+        spec = _rich_spec(name, grid, seed=13)
+    g, o = pair(spec)
+    got, ref = g.stray_field(height), o.stray_field(height)
+    assert field_err(got[:, None], ref[:, None]) < FIELD_TOL, name
+    assert np.abs(got[2] - ref[2]).max() < FIELD_TOL * np.abs(ref[2]).max()          # the imaged component, B_z
+    g.destroy()
+
+
+def test_stray_field_argument_errors_and_the_on_axis_closed_form():
+    """Periodic worlds are refused; the on-axis closed form of a uniformly magnetised square slab (P26a) on the CUDA path."""
+    spec = wl.make("c2", (16, 16, 1))
+    g = mmx.World.from_spec(spec, demag=False)
+    with pytest.raises(mmx.MmxError):
+        g.stray_field(10e-9)
+    g.destroy()
+    n, h, t, Ms, height = 21, 2e-9, 3e-9, 8e5, 60e-9
+    spec = wl.make("c1", (n, n, 1))
+    spec.cell, spec.demag = (h, h, t), False
+    spec.mat["Ms"][:] = Ms
+    m = np.zeros((3, 1, n, n), np.float32); m[2] = 1.0
+    spec.m = [m]
+    g = mmx.World.from_spec(spec)
+    B = g.stray_field(height)
+    a, zc = n * h, t / 2 + height
+    om = lambda d: 4 * np.arctan(a * a / (4 * d * np.sqrt(d * d + a * a / 2)))
+    want = 4e-7 * np.pi * Ms / (4 * np.pi) * (om(zc - t / 2) - om(zc + t / 2))
+    assert abs(B[2, n // 2, n // 2] - want) < 2e-3 * abs(want)
+    g.destroy()
