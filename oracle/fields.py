@@ -58,11 +58,14 @@ def _inv(ms):
 # ----------------------------------------------------------------------
 # Eq.3: exchange-like pair terms
 # ----------------------------------------------------------------------
-def pair_laplacian(mq, Ms, Apar, reg, scale, cell, pbc, factor):
+def pair_laplacian(mq, Ms, Apar, reg, scale, cell, pbc, factor, ghost=None):
     """sum over the 6 neighbours n of  factor * A_cn / Ms_c * (mq_n - mq_c) / h_n^2,
     A_cn = harmonic mean of Apar at c and n, times `scale` when c and n lie in
     different regions (S3, S4).  factor=2, mq=m^(s), Apar=A11: first term of Eq.3;
-    factor=1, mq=m^(s'), Apar=A12: second term (S5)."""
+    factor=1, mq=m^(s'), Apar=A12: second term (S5).
+    ghost: None = open boundary (S9: a pair whose partner is absent adds nothing); else a dict
+    (axis, d) -> ghost values of mq behind an absent partner (Neumann boundary of Eq.5, reading S41), which
+    then enter the pair with the centre cell's own Apar."""
     B = np.zeros_like(mq)
     iMs = _inv(Ms)
     for axis in range(3):
@@ -75,6 +78,9 @@ def pair_laplacian(mq, Ms, Apar, reg, scale, cell, pbc, factor):
             ok = ex & (Msn > 0) & (Ms > 0)
             Acn = _harmonic(Apar, An) * np.where(rn == reg, 1.0, scale)
             B += np.where(ok, factor * Acn * iMs / (h * h), 0.0)[None] * (mn - mq)
+            if ghost is not None:
+                absent = ~ok & (Ms > 0)
+                B += np.where(absent, factor * Apar * iMs / (h * h), 0.0)[None] * (ghost[(axis, d)] - mq)
     return B
 
 
@@ -96,7 +102,7 @@ def dmi_homogeneous(m_other, Ms, d, s):
     return B * _inv(Ms)[None]
 
 
-def dmi_tensor(mq, Ms, q, cell, pbc):
+def dmi_tensor(mq, Ms, q, cell, pbc, ghost=None):
     """General DMI of Eq.4 for s = s': eps = sum_ijk D_ijk m_j d_i m_k with
     D_ijk = -D_ikj, "9 independent components".  For each axis i the antisymmetric 3x3 block is a
     vector q_i, D_ijk = sum_l eps_jkl q_il, so eps = sum_i q_i . (m x d_i m) and
@@ -120,10 +126,13 @@ def dmi_tensor(mq, Ms, q, cell, pbc):
             ok = ex & (Msn > 0) & (Ms > 0)
             w = np.where(ok, iMs / h, 0.0) * d
             B += w[None] * cross(qv, mn)
+            if ghost is not None:   # Neumann boundary (reading S41): the absent partner is the ghost value
+                wg = np.where(~ok & (Ms > 0), iMs / h, 0.0) * d
+                B += wg[None] * cross(qv, ghost[(axis, d)])
     return B
 
 
-def dmi_interfacial(mq, Ms, D, cell, pbc):
+def dmi_interfacial(mq, Ms, D, cell, pbc, ghost=None):
     """B = sum_{n in +-x, +-y} D_cn / (Ms_c h_n) (z^ x e_cn) x mq_n ;
     continuum limit (2D/Ms)(dx m_z, dy m_z, -dx m_x - dy m_y)."""
     B = np.zeros_like(mq)
@@ -139,6 +148,10 @@ def dmi_interfacial(mq, Ms, D, cell, pbc):
             # (z^ x (d x^)) x m = d ( m_z, 0, -m_x);  (z^ x (d y^)) x m = d (0, m_z, -m_y)
             B[axis] += w * mn[2]
             B[2] -= w * mn[axis]
+            if ghost is not None:   # Neumann boundary (reading S41): ghost value, the centre cell's own D
+                wg = np.where(~ok & (Ms > 0), D * iMs / h, 0.0) * d
+                B[axis] += wg * ghost[(axis, d)][2]
+                B[2] -= wg * ghost[(axis, d)][axis]
     return B
 
 
@@ -244,3 +257,49 @@ def slonczewski_torque(m, Ms, alpha, gamma, pol, jz, mp, lam, eps_prime, thickne
     mxpxm = cross(m, pxm)
     pref = gamma * beta / (1.0 + alpha * alpha)
     return (pref * (eps + alpha * eps_prime))[None] * mxpxm + (pref * (eps_prime - alpha * eps))[None] * pxm
+
+
+# ----------------------------------------------------------------------
+# Eq.5: Neumann boundary condition as ghost cells -- reading S41
+# ----------------------------------------------------------------------
+def neumann_ghosts(m, A11, qn_of, A12, cell):
+    """Ghost values behind the six faces of every cell, for one or two sublattices.
+
+    Eq.5:  2 A11^(s) d_n m^(s) = A12 (d_n m^(s') x m^(s)) x m^(s) + D^(s).(n (x) m^(s)),  n the outward normal.
+    Readings (S41): (i) the contraction is the one the variation of Eq.4 fixes, D.(n (x) m) = m x q_n with
+    q_n = sum_i n_i q_i (interfacial D: q_x = D y^, q_y = -D x^), so that Eq.5 is the natural boundary condition
+    of the energy of Eq.3 + Eq.4; (ii) (a x m) x m = -(a - (a.m) m) = -P_m a, so for two sublattices the normal
+    derivatives g = d_n m, g' = d_n m' solve the linear system
+        2 A  g  + A12 P_m  g' = m  x q_n  = r
+        2 A' g' + A12 P_m' g  = m' x q'_n = r'
+    whose closed-form solution is, with w = P_m m', beta = A12^2/(2A'), R = r - (A12/2A') P_m r':
+        g.w = R.w / (2A - beta + beta |w|^2),   g = (R - beta (g.w) w)/(2A - beta),   g' = (r' - A12 P_m' g)/(2A');
+    one sublattice: g = r/(2A).  (iii) the ghost behind the face (axis i, side d) is m_c + h_i g (first order in h,
+    as mumax3 does for its DMI boundary), and enters every pair stencil in place of the absent partner.
+
+    m: list of S arrays [3,Nz,Ny,Nx]; A11: list of S per-cell arrays; qn_of(s, axis, d) -> [3,Nz,Ny,Nx] the vector
+    q_n = d q_axis of sublattice s per cell; A12 scalar.  Returns list over s of dict (axis, d) -> ghost array."""
+    S = len(m)
+    assert S <= 2, "Eq.5 is written for a sublattice s and its partner s'"
+    proj = lambda a, u: a - (a * u).sum(axis=0)[None] * u
+    out = [dict() for _ in range(S)]
+    for axis in range(3):
+        for d in (+1, -1):
+            r = [cross(m[s], qn_of(s, axis, d)) for s in range(S)]
+            iA = [np.where(A11[s] > 0, 1.0 / np.where(A11[s] > 0, 2.0 * A11[s], 1.0), 0.0) for s in range(S)]
+            if S == 1 or A12 == 0.0:
+                g = [iA[s][None] * r[s] for s in range(S)]
+            else:
+                g = [None, None]
+                a2, a2p = 2.0 * A11[0], 2.0 * A11[1]
+                beta = A12 * A12 * iA[1]
+                w = proj(m[1], m[0])
+                R = r[0] - (A12 * iA[1])[None] * proj(r[1], m[0])
+                den = a2 - beta
+                gw = (R * w).sum(axis=0) / (den + beta * (w * w).sum(axis=0))
+                g[0] = (R - (beta * gw)[None] * w) / den[None]
+                g[1] = iA[1][None] * (r[1] - A12 * proj(g[0], m[1]))
+                del a2p
+            for s in range(S):
+                out[s][(axis, d)] = m[s] + cell[axis] * g[s]
+    return out

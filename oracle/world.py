@@ -78,6 +78,23 @@ class World:
         return dm.stray_field_at_height(self.magnetisation(self.m if m is None else m), self.grid, self.cell, height,
                                         self.spec.cutoff_cells)
 
+    def ghosts(self, m):
+        """Ghost values of Eq.5's Neumann boundary condition for every sublattice (reading S41)."""
+        q = self.cpl.get("dmi_q")
+
+        def qn_of(s, axis, d):
+            D = self.p[s]["D"]
+            qa = np.zeros((3,) + D.shape)
+            if axis == 0:
+                qa[1] = D          # interfacial D: q_x = D y^
+            elif axis == 1:
+                qa[0] = -D         #                q_y = -D x^
+            if q is not None:
+                qa = qa + np.asarray(q, float)[s][axis].reshape(3, 1, 1, 1)
+            return d * qa
+
+        return fl.neumann_ghosts(m, [self.p[s]["A"] for s in range(self.S)], qn_of, float(self.cpl.get("A12", 0.0)), self.cell)
+
     # ------------------------------------------------------------------ fields
     def strain(self, u=None):
         u = self.u if u is None else u
@@ -92,14 +109,16 @@ class World:
         # first two" -- reading S38: the terms are summed over both partners)
         others = [t for t in range(self.S) if t != s]
         out = {}
+        gh = self.ghosts(m) if self.cpl.get("bc") == "neumann" else None   # Eq.5 (reading S41); None: open / periodic
+        G = (lambda t: None) if gh is None else (lambda t: gh[t])
         if terms & T_EXCH:
             out[T_EXCH] = fl.pair_laplacian(m[s], p["Ms"], p["A"], self.reg, self.cpl["scale_A11"],
-                                            self.cell, self.pbc, 2.0)
+                                            self.cell, self.pbc, 2.0, G(s))
         if terms & T_DMI:
-            out[T_DMI] = fl.dmi_interfacial(m[s], p["Ms"], p["D"], self.cell, self.pbc)
+            out[T_DMI] = fl.dmi_interfacial(m[s], p["Ms"], p["D"], self.cell, self.pbc, G(s))
             q = self.cpl.get("dmi_q")
             if q is not None and np.any(np.asarray(q)[s]):   # general tensor of Eq.4, same term bit
-                out[T_DMI] = out[T_DMI] + fl.dmi_tensor(m[s], p["Ms"], np.asarray(q)[s], self.cell, self.pbc)
+                out[T_DMI] = out[T_DMI] + fl.dmi_tensor(m[s], p["Ms"], np.asarray(q)[s], self.cell, self.pbc, G(s))
         if terms & T_ANIS_U:
             out[T_ANIS_U] = fl.uniaxial(m[s], p["Ms"], p["Ku1"], p["u"])
         if terms & T_ANIS_C:
@@ -112,13 +131,13 @@ class World:
             if terms & T_A12:
                 A12 = np.full_like(p["Ms"], self.cpl["A12"])
                 out[T_A12] = sum(fl.pair_laplacian(m[o], p["Ms"], A12, self.reg, self.cpl["scale_A12"],
-                                                   self.cell, self.pbc, 1.0) for o in others)
+                                                   self.cell, self.pbc, 1.0, G(o)) for o in others)
             if terms & T_A0:
                 out[T_A0] = sum(fl.homogeneous_exchange(m[o], p["Ms"], self.cpl["A0"], self.cpl["latcon"])
                                 for o in others)
             if terms & T_DMI_INTER:
                 Di = np.full_like(p["Ms"], self.cpl["D_inter"])
-                out[T_DMI_INTER] = sum(fl.dmi_interfacial(m[o], p["Ms"], Di, self.cell, self.pbc) for o in others)
+                out[T_DMI_INTER] = sum(fl.dmi_interfacial(m[o], p["Ms"], Di, self.cell, self.pbc, G(o)) for o in others)
                 q12 = self.cpl.get("dmi_q12")
                 if q12 is not None and np.any(np.asarray(q12)):
                     # Eq.4 with s != s' ("a third DMI tensor is used to describe the intersublattice
@@ -127,7 +146,7 @@ class World:
                     # expression with the partner's magnetisation (reading S33 for the tensor <-> q_i mapping)
                     for o in others:
                         out[T_DMI_INTER] = out[T_DMI_INTER] + fl.dmi_tensor(m[o], p["Ms"], np.asarray(q12, float),
-                                                                            self.cell, self.pbc)
+                                                                            self.cell, self.pbc, G(o))
             if terms & T_DMI_HOMO:
                 # Eq.6 between the pairs (first, second) of reading S32: (0,1) for two sublattices, the cyclic
                 # pairs (0,1), (1,2), (2,0) for three (reading S38); s is the first spin of the pair (s, s+1)

@@ -408,3 +408,90 @@ def test_P25_the_120_degree_state_closed_forms():
 
 
 GAMMA_ = 1.7595e11
+
+
+def _neumann_spec(grid, S, seed, pbc=(0, 0, 0)):
+    rng = np.random.default_rng(seed)
+    spec = wl.make("c3" if S == 2 else "c1", grid)
+    spec.pbc, spec.regions, spec.demag, spec.J = pbc, None, False, (0.0, 0.0, 0.0)
+    spec.cell = (2e-9, 2.5e-9, 1.5e-9)
+    spec.mat = wl.make_mat(S, Ms=np.array([[4e5], [7e5]])[:S], A=np.array([[1.0e-11], [0.8e-11]])[:S], alpha=0.1,
+                           D=np.array([[1.2e-3], [0.7e-3]])[:S])
+    spec.coupling = wl.default_coupling(A12=-3e-12 if S == 2 else 0.0, latcon=0.35e-9)
+    spec.coupling["dmi_q"] = 0.6e-3 * rng.standard_normal((S, 3, 3))
+    spec.coupling["bc"] = "neumann"
+    spec.m = [wl.random_unit(rng, grid) for _ in range(S)]
+    return spec
+
+
+def test_P27_neumann_ghosts_satisfy_eq5_as_printed():
+    """Eq.5 (P:L155-161) with the ghost derivatives g = d_n m, g' = d_n m' that oracle/fields.py::neumann_ghosts builds
+    its ghost cells from (reading S41):   2 A11 g = A12 (g' x m) x m + m x q_n   for both sublattices, every face,
+    the left side and the paper's double cross product written out here independently of the closed-form solve.
+    Special cases: one sublattice g = m x q_n/(2A); a collinear antiferromagnet (m' = -m, equal A and D) has g' = -g and
+    g = m x q_n/(2 A11 - A12)."""
+    from oracle import fields as fl
+    spec = _neumann_spec((5, 4, 3), 2, 9)
+    w = World(spec)
+    gh = w.ghosts(w.m)
+    q = np.asarray(spec.coupling["dmi_q"])
+    A12 = spec.coupling["A12"]
+    for axis in range(3):
+        for d in (+1, -1):
+            g = [(gh[s][(axis, d)] - w.m[s]) / spec.cell[axis] for s in range(2)]
+            for s in range(2):
+                o = 1 - s
+                qn = np.zeros((3,) + w.m[s].shape[1:])
+                if axis == 0:
+                    qn[1] = w.p[s]["D"]
+                elif axis == 1:
+                    qn[0] = -w.p[s]["D"]
+                qn = d * (qn + q[s][axis].reshape(3, 1, 1, 1))
+                lhs = 2 * w.p[s]["A"][None] * g[s]
+                rhs = A12 * fl.cross(fl.cross(g[o], w.m[s]), w.m[s]) + fl.cross(w.m[s], qn)
+                np.testing.assert_allclose(lhs, rhs, atol=1e-6 * np.abs(rhs).max())   # (|m| = 1 to fp32 rounding)
+                assert np.abs((g[s] * w.m[s]).sum(axis=0)).max() < 1e-9 * np.abs(g[s]).max()   # d_n m is tangent to the sphere
+    # collinear antiferromagnet
+    s2 = spec.copy()
+    s2.mat["A"][:], s2.mat["D"][:] = 1e-11, 1e-3
+    s2.coupling["dmi_q"] = None
+    s2.m = [spec.m[0], (-spec.m[0]).astype(np.float32)]
+    w = World(s2)
+    gh = w.ghosts(w.m)
+    qx = np.zeros_like(w.m[0]); qx[1] = 1e-3
+    g0 = (gh[0][(0, +1)] - w.m[0]) / s2.cell[0]
+    g1 = (gh[1][(0, +1)] - w.m[1]) / s2.cell[0]
+    np.testing.assert_allclose(g0, fl.cross(w.m[0], qx) / (2e-11 - A12), atol=1e-9 * np.abs(g0).max())
+    np.testing.assert_allclose(g1, -g0, atol=1e-9 * np.abs(g0).max())
+
+
+@pytest.mark.parametrize("hscale", [1.0, 0.25])
+def test_P27_neumann_minus_open_is_the_local_boundary_term(hscale):
+    """One sublattice: putting the ghost m_c + h d_n m behind an absent neighbour into the exchange AND the DMI pair
+    stencils, their O(1/h) parts cancel exactly (only then is the boundary condition the natural one of the energy of
+    Eq.3 + Eq.4 -- a ghost derivative wrong by any factor leaves a term that grows like 1/h) and what remains is
+        B_neumann - B_open = sum over absent neighbours (1/(2 A Ms)) q_i x (m_c x q_i),
+    independent of the cell size, = minus the gradient of the surface energy -(V/4A) |m x q_i|^2.  Checked on a random
+    3-D state at two cell sizes, q_i = interfacial + general tensor."""
+    from oracle import fields as fl
+    spec = _neumann_spec((5, 4, 3), 1, 19)
+    spec.cell = tuple(hscale * c for c in spec.cell)
+    so = spec.copy()
+    so.coupling["bc"] = "open"
+    wn, wo = World(spec), World(so)
+    diff = wn.heff(0, terms=T_EXCH | T_DMI) - wo.heff(0, terms=T_EXCH | T_DMI)
+    m, A, Ms, D = wn.m[0], 1.0e-11, 4e5, 1.2e-3
+    q = np.asarray(spec.coupling["dmi_q"])[0].copy()
+    q[0] += [0, D, 0]
+    q[1] += [-D, 0, 0]
+    want = np.zeros_like(m)
+    nx, ny, nz = spec.grid
+    for axis, n in ((0, nx), (1, ny), (2, nz)):
+        qv = q[axis].reshape(3, 1, 1, 1) * np.ones_like(m)
+        term = fl.cross(qv, fl.cross(m, qv)) / (2 * A * Ms)
+        for edge in (0, n - 1):
+            sl = [slice(None)] * 4
+            sl[3 - axis] = edge
+            want[tuple(sl)] += term[tuple(sl)]
+    np.testing.assert_allclose(diff, want, atol=1e-9 * np.abs(want).max())
+    assert np.abs(want).max() > 1e-3   # tesla: the term is not negligible at nm cell sizes
