@@ -189,6 +189,17 @@ int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]);
  * under the term bit MMX_T_DMI_INTER (two-sublattice worlds). */
 #define MMX_DMI_INTER (-1)
 
+/* Boundary condition on the non-periodic axes ("The Neumann boundary conditions as given in Eq. (5) are the
+ * default in mumax+.  Alternatively, open or periodic boundary conditions can be used").
+ *   MMX_BC_OPEN    a stencil pair whose partner is absent (outside the grid, or Ms = 0) adds nothing (reading S9; the
+ *                  natural boundary condition of the discrete pair energy; default of this library)
+ *   MMX_BC_NEUMANN Eq.5, 2 A11 d_n m = A12 (d_n m' x m) x m + D.(n (x) m), as ghost cells (reading S41): the absent partner of
+ *                  every exchange, A12 and DMI pair is m_c + h d_n m, with D.(n (x) m) = m x sum_i n_i q_i and the coupled
+ *                  two-sublattice system solved in closed form; it differs from MMX_BC_OPEN by the h-independent local term
+ *                  (1/(2 A Ms)) q_i x (m x q_i) on boundary cells (one sublattice).  One or two sublattices. */
+enum { MMX_BC_OPEN = 0, MMX_BC_NEUMANN = 1 };
+int mmx_set_boundary(mmx_world* w, int kind);
+
 /* Slonczewski spin-transfer torque ("as formulated by ... Slonczewski [29], implemented in the same way
  * as in mumax3"; reading S37).  A current density jz through the free layer (thickness d), polarised along
  * the fixed-layer direction mp, adds in Gilbert form  gamma beta [eps m x (mp x m) - eps' m x mp],

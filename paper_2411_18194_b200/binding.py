@@ -84,6 +84,7 @@ PROTOTYPES = {
     "mmx_set_bext": (C.c_int, [_W, _D3]),
     "mmx_set_current": (C.c_int, [_W, _D3]),
     "mmx_set_dmi_tensor": (C.c_int, [_W, C.c_int, C.POINTER(C.c_double)]),
+    "mmx_set_boundary": (C.c_int, [_W, C.c_int]),
     "mmx_set_slonczewski": (C.c_int, [_W, C.POINTER(Slonczewski)]),
     "mmx_set_elastic": (C.c_int, [_W, C.POINTER(Elastic)]),
     "mmx_enable_demag": (C.c_int, [_W, C.c_int]),
@@ -241,6 +242,10 @@ class World:
             return
         flat = [float(x) for x in np.asarray(q, dtype=np.float64).reshape(9)]
         _check(self.lib.mmx_set_dmi_tensor(self.h, int(sublattice), _arr(C.c_double, flat)))
+
+    def set_boundary(self, kind):
+        """kind: "open" (default) or "neumann" (Eq.5)."""
+        _check(self.lib.mmx_set_boundary(self.h, {"open": 0, "neumann": 1}[kind]))
 
     def set_slonczewski(self, jz=0.0, mp=(0.0, 0.0, 1.0), thickness=0.0, eps_prime=0.0, **kw):
         """Slonczewski torque parameters (keyword `lambda`: Slonczewski Lambda, default 1); jz = 0 clears."""
@@ -401,6 +406,7 @@ class World:
         dmi_q = cpl.pop("dmi_q", None)
         dmi_q12 = cpl.pop("dmi_q12", None)
         sl = cpl.pop("slonczewski", None)
+        bc = cpl.pop("bc", None)
         w.set_coupling(**cpl)
         if dmi_q is not None:
             for s in range(spec.S):
@@ -409,6 +415,8 @@ class World:
             w.set_dmi_tensor(DMI_INTER, np.asarray(dmi_q12))
         if sl:
             w.set_slonczewski(**sl)
+        if bc:
+            w.set_boundary(bc)
         w.set_bext(spec.bext)
         w.set_current(spec.J)
         if spec.elastic is not None:

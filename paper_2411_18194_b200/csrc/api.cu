@@ -269,6 +269,7 @@ void fill_local(const mmx_world* w, LocalArgs& a, unsigned terms) {
   a.terms = terms;
   a.has_J = (w->J[0] != 0.0 || w->J[1] != 0.0 || w->J[2] != 0.0) ? 1 : 0;
   a.relax = w->relax_mode ? 1 : 0;
+  a.neumann = w->boundary == MMX_BC_NEUMANN ? 1 : 0;
   a.bdemag = (terms & MMX_T_DEMAG) ? w->bdemag : nullptr;
   a.strain = (terms & MMX_T_MEL) ? w->strain : nullptr;
   a.ctrl = w->d_ctrl;
@@ -738,6 +739,17 @@ int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]) {
   w->has_dmiq = false;
   for (int s = 0; s < 4; ++s)
     for (int k = 0; k < 9; ++k) w->has_dmiq = w->has_dmiq || w->dmiq[s][k] != 0.0;
+  w->k1_valid = false;
+  w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
+  return MMX_OK;
+}
+
+int mmx_set_boundary(mmx_world* w, int kind) {
+  if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
+  if (kind != MMX_BC_OPEN && kind != MMX_BC_NEUMANN) return mmx_fail(MMX_EINVAL, "unknown boundary kind %d", kind);
+  if (kind == MMX_BC_NEUMANN && w->S > 2)
+    return mmx_fail(MMX_EINVAL, "the Neumann boundary condition of Eq.5 is written for one sublattice and its partner");
+  w->boundary = kind;
   w->k1_valid = false;
   w->cfg_epoch++;  // kernel arguments change: the captured step graph is stale
   return MMX_OK;

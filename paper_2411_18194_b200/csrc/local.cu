@@ -85,6 +85,39 @@ __device__ __forceinline__ long long nbr(const LocalArgs& a, int ix, int iy, int
   return ((long long)p[2] * a.ny + p[1]) * a.nx + p[0];
 }
 
+// Neumann boundary condition of Eq.5 as ghost cells, reading S41: normal derivatives g = d_n m of sublattice
+// s and (two sublattices) of its partner o at a face with outward normal d e_axis, from
+//     2 A g + A12 P_m g' = m x q_n,   2 A' g' + A12 P_m' g = m' x q'_n,   q_n = d (q_axis + interfacial part)
+// solved in closed form (w = P_m m', beta = A12^2/(2A'), R = r - (A12/2A') P_m r'):
+//     g.w = R.w/(2A - beta + beta |w|^2),  g = (R - beta (g.w) w)/(2A - beta),  g' = (r' - A12 P_m' g)/(2A').
+__device__ __forceinline__ V3 qn_of(const LocalArgs& a, int s, int axis, float d, float Dc) {
+  V3 q = v3(a.dmiq[s][axis][0], a.dmiq[s][axis][1], a.dmiq[s][axis][2]);
+  if (axis == 0) q.y += Dc;        // interfacial D: q_x = D y^
+  else if (axis == 1) q.x -= Dc;   //                q_y = -D x^
+  return d * q;
+}
+__device__ __forceinline__ V3 perp(V3 v, V3 u) { return v - dot(v, u) * u; }
+__device__ __forceinline__ void neumann_g(const LocalArgs& a, bool two, int s, int o, int axis, float d, V3 ms, V3 mo,
+                                          const float* Ps, const float* Po, V3& gs, V3& go) {
+  const float A = Ps[MP_A];
+  const V3 r = cross(ms, qn_of(a, s, axis, d, Ps[MP_D]));
+  gs = go = v3(0.f, 0.f, 0.f);
+  if (!(A > 0.f)) return;
+  if (!two || a.A12 == 0.f || !(Po[MP_A] > 0.f)) {
+    gs = (0.5f / A) * r;
+    if (two && Po[MP_A] > 0.f) go = (0.5f / Po[MP_A]) * cross(mo, qn_of(a, o, axis, d, Po[MP_D]));
+    return;
+  }
+  const float iAp = 0.5f / Po[MP_A];
+  const V3 rp = cross(mo, qn_of(a, o, axis, d, Po[MP_D]));
+  const float beta = a.A12 * a.A12 * iAp, den = 2.f * A - beta;
+  const V3 w = perp(mo, ms);
+  const V3 R = r - (a.A12 * iAp) * perp(rp, ms);
+  const float gw = dot(R, w) / (den + beta * dot(w, w));
+  gs = (1.f / den) * (R - (beta * gw) * w);
+  go = iAp * (rp - a.A12 * perp(gs, mo));
+}
+
 template <int S, bool REG>
 __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
   MmxCtrl* ctrl = a.ctrl;
@@ -170,6 +203,38 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
                     B = fma3(iMs * a.inv_h[axis] * d, cross(qv, on), B);
                   }
                 }
+              }
+            }
+          }
+          if (a.neumann && S <= 2 && !(ni[q] >= 0 && (REG ? a.mat[((size_t)s * a.nreg + rn[q]) * MMX_MATW + MP_MS] : Ms) > 0.f)) {
+            // absent partner: Neumann ghost m_c + h d_n m in every pair stencil, the centre cell's own constants
+            const int o = S == 2 ? 1 - s : s;
+            const float* Po = a.mat + ((size_t)o * a.nreg + rc) * MMX_MATW;
+            V3 gs, go;
+            neumann_g(a, S == 2, s, o, axis, d, mc[s], mc[o], P, Po, gs, go);
+            const float h = 1.f / a.inv_h[axis];
+            const V3 mg = fma3(h, gs, mc[s]);
+            if (a.terms & MMX_T_EXCH) B = fma3(2.f * Ac * iMs * a.inv_h2[axis], mg - mc[s], B);
+            if (axis < 2 && (a.terms & MMX_T_DMI)) {
+              const float wd = Dc * iMs * a.inv_h[axis] * d;
+              if (axis == 0) { B.x = fmaf(wd, mg.z, B.x); B.z = fmaf(-wd, mg.x, B.z); }
+              else { B.y = fmaf(wd, mg.z, B.y); B.z = fmaf(-wd, mg.y, B.z); }
+            }
+            if (a.has_dmiq && (a.terms & MMX_T_DMI)) {
+              const V3 qv = v3(a.dmiq[s][axis][0], a.dmiq[s][axis][1], a.dmiq[s][axis][2]);
+              B = fma3(iMs * a.inv_h[axis] * d, cross(qv, mg), B);
+            }
+            if (S == 2 && (a.terms & (MMX_T_A12 | MMX_T_DMI_INTER))) {
+              const V3 og = fma3(h, go, mc[o]);
+              if (a.terms & MMX_T_A12) B = fma3(a.A12 * iMs * a.inv_h2[axis], og - mc[o], B);
+              if (axis < 2 && (a.terms & MMX_T_DMI_INTER)) {
+                const float wd = a.Dinter * iMs * a.inv_h[axis] * d;
+                if (axis == 0) { B.x = fmaf(wd, og.z, B.x); B.z = fmaf(-wd, og.x, B.z); }
+                else { B.y = fmaf(wd, og.z, B.y); B.z = fmaf(-wd, og.y, B.z); }
+              }
+              if (a.has_dmiq12 && (a.terms & MMX_T_DMI_INTER)) {
+                const V3 qv = v3(a.dmiq[3][axis][0], a.dmiq[3][axis][1], a.dmiq[3][axis][2]);
+                B = fma3(iMs * a.inv_h[axis] * d, cross(qv, og), B);
               }
             }
           }
@@ -974,8 +1039,8 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   const unsigned blocks = (unsigned)((N + 255) / 256);
   const bool reg = w->nreg > 1;
   ProfScope ps(w, PK_LOCAL);
-  // (the general DMI tensors and the Slonczewski torque live in the general kernel k_local only)
-  bool uniform = !reg && (w->grid[0] % 4) == 0 && !a.has_dmiq && !a.has_sl;
+  // (the general DMI tensors, the Slonczewski torque and the Neumann boundary live in the general kernel k_local only)
+  bool uniform = !reg && (w->grid[0] % 4) == 0 && !a.has_dmiq && !a.has_sl && !a.neumann;
   for (int s = 0; s < w->S && uniform; ++s) uniform = w->mats[(size_t)s * w->nreg].Ms > 0;
   if (w->S > 2) uniform = false;  // (three sublattices: general kernel)
   const bool open_all = !a.per[0] && !a.per[1] && !a.per[2];

@@ -74,6 +74,7 @@ struct LocalArgs {
   unsigned terms;
   int has_J;
   int relax;             // 1: damping-only torque (mmx_relax, reading S39)
+  int neumann;           // 1: Neumann boundary condition of Eq.5 (ghost cells, reading S41); 0: open (S9)
   // inputs.  A "sel pair" p[2] is indexed with ctrl->sel inside the kernel.
   const float* yin[2];     // stage state [nvec][3][N]
   const float* bdemag;     // [3][N] or null
@@ -171,6 +172,7 @@ struct mmx_world {
   double dmiq[4][9];   // general DMI tensors (mmx_set_dmi_tensor): sublattice 0, 1, 2, inter-sublattice; zero = none
   bool has_dmiq;
   mmx_slonczewski sl;  // jz = 0: off
+  int boundary;        // MMX_BC_OPEN / MMX_BC_NEUMANN (non-periodic axes)
   bool relax_mode;     // stepping inside mmx_relax: the local kernels drop the precession term
   bool has_elastic;
   mmx_elastic el;

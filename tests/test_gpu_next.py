@@ -263,3 +263,50 @@ def test_stray_field_argument_errors_and_the_on_axis_closed_form():
     want = 4e-7 * np.pi * Ms / (4 * np.pi) * (om(zc - t / 2) - om(zc + t / 2))
     assert abs(B[2, n // 2, n // 2] - want) < 2e-3 * abs(want)
     g.destroy()
+
+
+@pytest.mark.parametrize("name,grid,pbc", [("c1", (24, 12, 1), (0, 0, 0)), ("c4", (12, 10, 5), (0, 0, 0)), ("c3", (32, 16, 1), (0, 0, 0)),
+                                           ("c3", (24, 16, 2), (0, 2, 0))])
+def test_neumann_boundary_condition(name, grid, pbc):
+    """Eq.5, the paper's default boundary condition, reading S41: ghost cells in the exchange, A12 and DMI
+    pairs (interfacial + general tensors), one and two sublattices, grains and holes (a cell next to an empty cell is a
+    boundary cell), mixed periodic / Neumann axes: each term, the total field, torque, energy and a short trajectory
+    against the oracle; the boundary condition must matter."""
+    spec = _rich_spec(name, grid, seed=43)
+    spec.pbc = pbc
+    rng = np.random.default_rng(47)
+    spec.coupling["dmi_q"] = 0.8e-3 * rng.standard_normal((spec.S, 3, 3))
+    if spec.S == 2:
+        spec.coupling["dmi_q12"] = 0.5e-3 * rng.standard_normal((3, 3))
+        spec.mat["Ms"][:, 3] = 0.0                      # one grain is empty: its neighbours see a boundary
+    spec.coupling["bc"] = "neumann"
+    g, o = pair(spec)
+    so = spec.copy()
+    so.coupling["bc"] = "open"
+    from gpu_util import pair_oracle
+    o_open = pair_oracle(so)
+    bits = [mmx.T_EXCH, mmx.T_DMI] + ([mmx.T_A12, mmx.T_DMI_INTER] if spec.S == 2 else [])
+    for s in range(spec.S):
+        mag = (o.p[s]["Ms"] > 0)[None]
+        ref = o.field_terms(s)
+        assert field_err(o_open.heff(s) * mag, o.heff(s) * mag) > 1e-3
+        for bit in bits:
+            assert field_err(g.eval_heff(s, bit), ref[bit] * mag) < FIELD_TOL, (name, s, bit)
+        B = o.heff(s) * mag
+        if spec.demag:
+            B = B - ref[oc.T_DEMAG] * (~mag)               # (library convention S35: B_eff = 0 in empty cells)
+        assert field_err(g.eval_heff(s, mmx.T_ALL), o.heff(s) * mag) < FIELD_TOL, (name, s)
+        assert field_err(g.eval_torque(s), o.torque(s)) < FIELD_TOL, (name, s)
+    Eg, Eo = g.energy(mmx.T_EXCH | mmx.T_DMI), o.energy(oc.T_EXCH | oc.T_DMI)
+    assert abs(Eg - Eo) < 1e-5 * abs(Eo)
+    dt = spec.integrator["dt"]
+    g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=20)
+    o.step_dp45_fixed(dt, 20)
+    for s in range(spec.S):
+        assert max_dm(g.get_state(mmx.F_M[s]), o.m[s]) <= TRAJ_TOL
+    g.set_boundary("open")
+    for s in range(spec.S):
+        g.set_state(mmx.F_M[s], np.ascontiguousarray(spec.m[s], dtype=np.float32))
+    mag = (o.p[0]["Ms"] > 0)[None]
+    assert field_err(g.eval_heff(0, mmx.T_EXCH | mmx.T_DMI), o_open.heff(0, terms=oc.T_EXCH | oc.T_DMI) * mag) < FIELD_TOL
+    g.destroy()
