@@ -301,15 +301,42 @@ struct CtrlHost {  // leading part of MmxCtrl, up to (not including) ca
   MmxCtrl c;
 };
 
+// The leading part of the controller block (everything before the coefficient tables) travels between host and
+// device without the copy engines: a write is a one-thread kernel that takes the words as its parameter, a read is a
+// one-warp kernel that stores them into mapped pinned host memory.  A stepping call therefore never queues behind a
+// caller's bulk cudaMemcpyAsync on another stream (the end-to-end leg of bench.py overlaps 50 MB copies with the step).
+constexpr int CTRL_HEAD_WORDS = (int)(offsetof(MmxCtrl, ca) / sizeof(unsigned));
+struct CtrlHead {
+  unsigned w[CTRL_HEAD_WORDS];
+};
+__global__ void k_ctrl_put(MmxCtrl* c, CtrlHead h) {
+  unsigned* dst = reinterpret_cast<unsigned*>(c);
+  for (int i = threadIdx.x; i < CTRL_HEAD_WORDS; i += blockDim.x) dst[i] = h.w[i];
+}
+__global__ void k_ctrl_get(const MmxCtrl* c, unsigned* host_mapped) {
+  const unsigned* src = reinterpret_cast<const unsigned*>(c);
+  for (int i = threadIdx.x; i < CTRL_HEAD_WORDS; i += blockDim.x) host_mapped[i] = src[i];
+  __threadfence_system();
+}
+
 int read_ctrl(mmx_world* w, MmxCtrl* h) {
-  MMX_CUDA(cudaMemcpyAsync(h, w->d_ctrl, offsetof(MmxCtrl, ca), cudaMemcpyDeviceToHost, w->stream));
+  if (!w->h_ctrl) {
+    MMX_CUDA(cudaMemcpyAsync(h, w->d_ctrl, offsetof(MmxCtrl, ca), cudaMemcpyDeviceToHost, w->stream));
+    MMX_CUDA(cudaStreamSynchronize(w->stream));
+    return MMX_OK;
+  }
+  k_ctrl_get<<<1, 32, 0, w->stream>>>(w->d_ctrl, w->h_ctrl);
+  MMX_CUDA(cudaGetLastError());
   MMX_CUDA(cudaStreamSynchronize(w->stream));
+  memcpy(h, w->h_ctrl, offsetof(MmxCtrl, ca));
   return MMX_OK;
 }
 
 int write_ctrl(mmx_world* w, const MmxCtrl* h) {
-  MMX_CUDA(cudaMemcpyAsync(w->d_ctrl, h, offsetof(MmxCtrl, ca), cudaMemcpyHostToDevice, w->stream));
-  MMX_CUDA(cudaStreamSynchronize(w->stream));
+  CtrlHead hd;
+  memcpy(hd.w, h, offsetof(MmxCtrl, ca));
+  k_ctrl_put<<<1, 32, 0, w->stream>>>(w->d_ctrl, hd);
+  MMX_CUDA(cudaGetLastError());
   return MMX_OK;
 }
 
@@ -622,7 +649,7 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
   w->Y[0] = w->Y[1] = w->YS[0] = w->YS[1] = nullptr;
   for (int i = 0; i <= MMX_MAX_STAGES; ++i) w->K[i] = nullptr;
   w->bdemag = w->strain = w->strain_f = w->scratch = nullptr;
-  w->d_ctrl = nullptr; w->d_acc = nullptr;
+  w->d_ctrl = nullptr; w->d_acc = nullptr; w->h_ctrl = nullptr;
   w->sel_host = 0; w->k1_valid = false; w->k1_method = -1;
   w->dev_bytes = 0; w->launches = 0;
   w->prof = false;
@@ -640,6 +667,10 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
       if (e != cudaSuccess) rc = mmx_fail(MMX_ECUDA, "ctrl upload failed: %s", cudaGetErrorString(e));
     }
   }
+  if (!rc && cudaHostAlloc(reinterpret_cast<void**>(&w->h_ctrl), offsetof(MmxCtrl, ca), cudaHostAllocMapped) != cudaSuccess) {
+    cudaGetLastError();
+    w->h_ctrl = nullptr;  // (read_ctrl falls back to a plain copy)
+  }
   if (rc) { mmx_world_destroy(w); return rc; }
   *out = w;
   return MMX_OK;
@@ -649,6 +680,7 @@ int mmx_world_destroy(mmx_world* w) {
   if (!w) return MMX_OK;
   cudaStreamSynchronize(w->stream);
   cudaFree(w->d_reg); cudaFree(w->d_mat); cudaFree(w->d_ctrl); cudaFree(w->d_acc);
+  if (w->h_ctrl) cudaFreeHost(w->h_ctrl);
   for (int i = 0; i < 2; ++i) { cudaFree(w->Y[i]); cudaFree(w->YS[i]); }
   for (int i = 0; i <= MMX_MAX_STAGES; ++i) cudaFree(w->K[i]);
   cudaFree(w->bdemag); cudaFree(w->strain); cudaFree(w->strain_f); cudaFree(w->scratch);

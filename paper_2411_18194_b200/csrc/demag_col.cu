@@ -356,14 +356,18 @@ __global__ void __launch_bounds__(2 * R * TILE, 2) k_mid_col(MidColArgs a) {
 // cp.async while the current tile is transformed; the halves of the inverse meet by shuffle.
 // Small CTAs (16 R threads, 65-97 KB) so that three (forward) or two (inverse) of them share an SM.
 // (two CTAs of 128 registers per SM beat three of 80 once the twiddles are register-resident)
+#ifndef MMX_MIDP_FWD_STAGES
+#define MMX_MIDP_FWD_STAGES 2
+#endif
 template <int R, int DIR>
 __global__ void __launch_bounds__(16 * R, 2) k_mid_pipe(MidColArgs a) {
   constexpr int H = R * R, P = 2 * H, TL = 8, NT = 16 * R;
   constexpr int ROWS = DIR < 0 ? H : P;   // rows of a staged tile
+  constexpr int NSTG = DIR < 0 ? MMX_MIDP_FWD_STAGES : 2;   // cp.async stages (tiles in flight + the one being transformed)
   constexpr int EXT = H * TL + 8;         // exchange tile of one half (+8: the halves use different banks)
   extern __shared__ __align__(16) unsigned char smraw[];
   float2* exb = reinterpret_cast<float2*>(smraw);   // [2][EXT]
-  float2* stage = exb + 2 * EXT;                     // [2][ROWS][TL]
+  float2* stage = exb + 2 * EXT;                     // [NSTG][ROWS][TL]
   __shared__ float2 stw[P];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int kxl = lane & 7, h = (lane >> 3) & 1, j = 2 * wid + (lane >> 4);
@@ -424,16 +428,19 @@ __global__ void __launch_bounds__(16 * R, 2) k_mid_pipe(MidColArgs a) {
   };
 
   int tile = blockIdx.x;
-  if (tile < nt) issue(tile, 0);
+  // prologue: NSTG - 1 tiles in flight (an empty group keeps the group count uniform past the end)
+#pragma unroll
+  for (int p = 0; p < NSTG - 1; ++p) {
+    if (tile + p * (int)gridDim.x < nt) issue(tile + p * gridDim.x, p);
+    else asm volatile("cp.async.commit_group;" ::: "memory");
+  }
   int buf = 0;
-  for (; tile < nt; tile += gridDim.x, buf ^= 1) {
-    const int nxt = tile + gridDim.x;
-    if (nxt < nt) {
-      issue(nxt, buf ^ 1);
-      asm volatile("cp.async.wait_group 1;" ::: "memory");
-    } else {
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
-    }
+  for (; tile < nt; tile += gridDim.x, buf = (buf + 1 == NSTG ? 0 : buf + 1)) {
+    const int nxt = tile + (NSTG - 1) * gridDim.x;
+    // (the stage refilled here was read before the block barriers of the previous iteration)
+    if (nxt < nt) issue(nxt, buf == 0 ? NSTG - 1 : buf - 1);
+    else asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group %0;" ::"n"(NSTG - 1) : "memory");
     __syncthreads();  // tile landed for all threads; exchange tiles of the previous tile are free
     int kx, slab;
     bool ok = true;
@@ -573,7 +580,7 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
     if (b.nyq) { b.ntile_main = (a.xc - 1) / TL; b.xc_main = a.xc - 1; }
     else { b.ntile_main = (a.xc + TL - 1) / TL; b.xc_main = a.xc; }
     const int nt = b.ntile_main * a.nslab + (b.nyq ? (a.nslab + TL - 1) / TL : 0);
-    const size_t sm = sizeof(float2) * (2 * (R * R * TL + 8) + 2 * (dir < 0 ? R * R : 2 * R * R) * TL);
+    const size_t sm = sizeof(float2) * (2 * (R * R * TL + 8) + (dir < 0 ? MMX_MIDP_FWD_STAGES * R * R : 2 * 2 * R * R) * TL);
     if (dir < 0) {
       if (int rc = set_smem_col(k_mid_pipe<16, -1>, sm)) return rc;
       int grid = mmx_persistent_grid(k_mid_pipe<16, -1>, 16 * 16, sm, w->sm_count, 2);

@@ -187,6 +187,7 @@ struct mmx_world {
   float* strain_f;     // [6][N], only with viscous elastic damping
   float* scratch;      // [3][N]
   MmxCtrl* d_ctrl;
+  unsigned* h_ctrl;    // mapped pinned host copy of the controller block's leading part (read_ctrl in api.cu)
   double* d_acc;       // fp64 accumulators for energies
   int sel_host;        // mirror of ctrl->sel valid when host_sel_valid
   bool k1_valid;       // FSAL k1 matches the current state
