@@ -356,14 +356,11 @@ __global__ void __launch_bounds__(2 * R * TILE, 2) k_mid_col(MidColArgs a) {
 // cp.async while the current tile is transformed; the halves of the inverse meet by shuffle.
 // Small CTAs (16 R threads, 65-97 KB) so that three (forward) or two (inverse) of them share an SM.
 // (two CTAs of 128 registers per SM beat three of 80 once the twiddles are register-resident)
-#ifndef MMX_MIDP_FWD_STAGES
-#define MMX_MIDP_FWD_STAGES 2
-#endif
 template <int R, int DIR>
 __global__ void __launch_bounds__(16 * R, 2) k_mid_pipe(MidColArgs a) {
   constexpr int H = R * R, P = 2 * H, TL = 8, NT = 16 * R;
   constexpr int ROWS = DIR < 0 ? H : P;   // rows of a staged tile
-  constexpr int NSTG = DIR < 0 ? MMX_MIDP_FWD_STAGES : 2;   // cp.async stages (tiles in flight + the one being transformed)
+  constexpr int NSTG = 2;   // cp.async stages (a third forward stage was measured: 70.3 vs 69.1 us, no gain)
   constexpr int EXT = H * TL + 8;         // exchange tile of one half (+8: the halves use different banks)
   extern __shared__ __align__(16) unsigned char smraw[];
   float2* exb = reinterpret_cast<float2*>(smraw);   // [2][EXT]
@@ -580,7 +577,7 @@ static int mid_col_launch_t(mmx_world* w, MidColArgs& a, int dir) {
     if (b.nyq) { b.ntile_main = (a.xc - 1) / TL; b.xc_main = a.xc - 1; }
     else { b.ntile_main = (a.xc + TL - 1) / TL; b.xc_main = a.xc; }
     const int nt = b.ntile_main * a.nslab + (b.nyq ? (a.nslab + TL - 1) / TL : 0);
-    const size_t sm = sizeof(float2) * (2 * (R * R * TL + 8) + (dir < 0 ? MMX_MIDP_FWD_STAGES * R * R : 2 * 2 * R * R) * TL);
+    const size_t sm = sizeof(float2) * (2 * (R * R * TL + 8) + 2 * (dir < 0 ? R * R : 2 * R * R) * TL);
     if (dir < 0) {
       if (int rc = set_smem_col(k_mid_pipe<16, -1>, sm)) return rc;
       int grid = mmx_persistent_grid(k_mid_pipe<16, -1>, 16 * 16, sm, w->sm_count, 2);
