@@ -407,6 +407,29 @@ def run_mmx(args, rank, local_rank, world_size):
     dev_bytes = g.device_bytes()
     g.destroy()
 
+    # ---- the other BASELINE.json configs (parity cases, small 2-D grids that fit in L2): DP45 fixed dt, same timing
+    # rules, reported beside the headline (they are latency-bound: DESIGN.md section 8)
+    others = None
+    if rank == 0 and world_size == 1 and name == "c4" and not args.no_other_configs:
+        others = {}
+        for oname in ("c1", "c2", "c3", "c5"):
+            ospec = wl.make(oname)
+            og = mmx.World.from_spec(ospec, stream=stream.cuda_stream)
+            run = lambda n: og.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=DT[oname], nsteps=n)
+            run(5)
+            ko = 100
+            o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            o0.record(stream)
+            run(ko)
+            o1.record(stream)
+            torch.cuda.synchronize()
+            oms = o0.elapsed_time(o1) / ko
+            others[oname] = {"grid": list(ospec.grid), "S": ospec.S, "ms_per_step": oms, "steps_per_s": 1e3 / oms,
+                             "cell_updates_per_s": ospec.ncells * 1e3 / oms,
+                             "frac_of_8TBs_survey_model": survey_step_bytes(ospec) / (oms * 1e-3) / 8e12}
+            og.destroy()
+
     cpu = None
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
         grid = oracle_sample_grid(name, 1)
@@ -423,7 +446,7 @@ def run_mmx(args, rank, local_rank, world_size):
             "config": {"workload": "%s %dx%dx%d DP45 fixed dt=%g, demag+exchange" % (name, *spec.grid, dt),
                        "cells": N, "field_evals_per_s": value * 6,
                        "l2": "working set %.2f GB >> 126 MB L2, no flush needed" % (dev_bytes / 1e9),
-                       "parallelism": "replicas x%d" % world_size},
+                       "parallelism": "replicas x%d" % world_size, "other_configs": others},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
             "cpu_baseline": cpu, "adaptive": adaptive,
         }
@@ -440,6 +463,7 @@ def main():
     ap.add_argument("--impl", default="mmx", choices=["mmx", "reference"])
     ap.add_argument("--config", default="c4", choices=list(DT))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
