@@ -25,10 +25,14 @@ using namespace mmxfft;
 
 namespace {
 
+// lines (rows / columns) of a CTA tile: "wide" tiles for grids that fill the GPU anyway, "narrow" ones (an eighth) for
+// small grids, where the number of CTAs -- not the width of a CTA's memory accesses -- decides the time of a pass
+// (c2's inner pass ran on 9 CTAs with wide tiles)
 constexpr int lines_for(int P) {
   return P <= 256 ? 16 : (4096 / P < 2 ? 2 : 4096 / P);
 }
-constexpr int block_for(int P) { return lines_for(P) * threads_per_line(P); }
+constexpr int lines_narrow(int P) { return lines_for(P) / 8 < 1 ? 1 : lines_for(P) / 8; }
+constexpr int block_of(int P, int L) { return L * threads_per_line(P); }
 
 struct XArgs {
   int nx, rows, xc, xp, S, nreg, gated;
@@ -73,9 +77,9 @@ __device__ __forceinline__ float gather_M(const XArgs& a, const float* y, size_t
   return M;
 }
 
-template <int P>
-__global__ void __launch_bounds__(block_for(P)) k_x_fwd(XArgs a) {
-  constexpr int L = lines_for(P), LP = L | 1, TPL = threads_per_line(P);
+template <int P, int L>
+__global__ void __launch_bounds__(block_of(P, L)) k_x_fwd(XArgs a) {
+  constexpr int LP = L | 1, TPL = threads_per_line(P);
   extern __shared__ float2 s[];
   if (a.gated && !a.ctrl->active) return;
   const float* y = a.yin[a.ctrl->sel];
@@ -115,9 +119,9 @@ __global__ void __launch_bounds__(block_for(P)) k_x_fwd(XArgs a) {
   }
 }
 
-template <int P>
-__global__ void __launch_bounds__(block_for(P)) k_x_inv(XArgs a) {
-  constexpr int L = lines_for(P), LP = L | 1, TPL = threads_per_line(P);
+template <int P, int L>
+__global__ void __launch_bounds__(block_of(P, L)) k_x_inv(XArgs a) {
+  constexpr int LP = L | 1, TPL = threads_per_line(P);
   extern __shared__ float2 s[];
   if (a.gated && !a.ctrl->active) return;
   const int tid = threadIdx.x, T = L * TPL;
@@ -143,9 +147,9 @@ __global__ void __launch_bounds__(block_for(P)) k_x_inv(XArgs a) {
   }
 }
 
-template <int P, int DIR>
-__global__ void __launch_bounds__(block_for(P)) k_mid(MidArgs a) {
-  constexpr int L = lines_for(P), LP = L, TPL = threads_per_line(P);
+template <int P, int L, int DIR>
+__global__ void __launch_bounds__(block_of(P, L)) k_mid(MidArgs a) {
+  constexpr int LP = L, TPL = threads_per_line(P);
   extern __shared__ float2 s[];
   if (a.gated && !a.ctrl->active) return;
   const int tid = threadIdx.x, T = L * TPL;
@@ -166,9 +170,9 @@ __global__ void __launch_bounds__(block_for(P)) k_mid(MidArgs a) {
   }
 }
 
-template <int P>
-__global__ void __launch_bounds__(block_for(P)) k_inner(InnerArgs a) {
-  constexpr int L = lines_for(P), LP = L, TPL = threads_per_line(P);
+template <int P, int L>
+__global__ void __launch_bounds__(block_of(P, L)) k_inner(InnerArgs a) {
+  constexpr int LP = L, TPL = threads_per_line(P);
   extern __shared__ float2 s[];
   if (a.gated && !a.ctrl->active) return;
   const int tid = threadIdx.x, T = L * TPL;
@@ -297,6 +301,12 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
   DemagPlan& d = w->dm;
   if (!d.ready) return mmx_fail(MMX_ESTATE, "mmx_demag_kernel_init has not been called");
   cudaStream_t st = w->stream;
+  // narrow CTA tiles when the wide ones would leave most of the GPU idle.  Measured (c1, c2, c3, c5):
+  // the row passes gain whenever the wide grid has fewer CTAs than multiprocessors (c5 x forward 18.4 -> 14.8 us with
+  // 48 -> 192 CTAs), the column passes only when it has fewer than a quarter of them (c2 inner 21.0 -> 16.8 us with
+  // 9 -> 65 CTAs; c3 with 65 wide CTAs lost 2 us on narrow 32-byte column accesses)
+  auto narrow_rows = [&](long long ctas_wide) { return ctas_wide < (long long)w->sm_count; };
+  auto narrow = [&](long long ctas_wide) { return 4 * ctas_wide < (long long)w->sm_count; };
   const int rows = 3 * d.nz * d.ny;
   const bool three_d = d.nz > 1;
   XArgs xa;
@@ -305,14 +315,15 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
   xa.reg = w->nreg > 1 ? w->d_reg : nullptr; xa.mat = w->d_mat; xa.ctrl = w->d_ctrl;
   xa.tw = d.tw[0]; xa.spec = d.spec1; xa.bout = bout;
 
-#define CALL_XF(PP)                                                                       \
+#define CALL_XF_L(PP, L)                                                                  \
   {                                                                                       \
-    constexpr int L = lines_for(PP);                                                      \
     size_t sm = sizeof(float2) * PP * (L | 1);                                            \
-    if (int rc = set_smem(k_x_fwd<PP>, sm)) return rc;                                    \
+    if (int rc = set_smem(k_x_fwd<PP, L>, sm)) return rc;                                 \
     ProfScope ps(w, PK_X_FWD);                                                             \
-    k_x_fwd<PP><<<(rows + 2 * L - 1) / (2 * L), block_for(PP), sm, st>>>(xa);             \
+    k_x_fwd<PP, L><<<(rows + 2 * L - 1) / (2 * L), block_of(PP, L), sm, st>>>(xa);        \
   }
+#define CALL_XF(PP)                                                                       \
+  if (narrow_rows((rows + 2 * lines_for(PP) - 1) / (2 * lines_for(PP)))) CALL_XF_L(PP, lines_narrow(PP)) else CALL_XF_L(PP, lines_for(PP))
   const bool xwarp = mmx_x_warp_ok(w);
   if (xwarp) {
     if (int rc = mmx_x_warp_launch(w, -1, yin, bout)) return rc;
@@ -326,15 +337,16 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ma.n_in = d.ny; ma.n_out = d.py; ma.xc = d.xc; ma.xp = d.xp; ma.gated = 1;
     ma.in_outer = (size_t)d.ny * d.xp; ma.out_outer = (size_t)d.py * d.xp;
     ma.in = d.spec1; ma.out = d.spec2; ma.tw = d.tw[1]; ma.ctrl = w->d_ctrl;
-#define CALL_MF(PP)                                                                       \
+#define CALL_MF_L(PP, L)                                                                  \
   {                                                                                       \
-    constexpr int L = lines_for(PP);                                                      \
     size_t sm = sizeof(float2) * PP * L;                                                  \
-    if (int rc = set_smem(k_mid<PP, -1>, sm)) return rc;                                  \
+    if (int rc = set_smem(k_mid<PP, L, -1>, sm)) return rc;                               \
     dim3 g((d.xc + L - 1) / L, 3 * d.nz);                                                 \
     ProfScope ps(w, PK_MID_FWD);                                                           \
-    k_mid<PP, -1><<<g, block_for(PP), sm, st>>>(ma);                                      \
+    k_mid<PP, L, -1><<<g, block_of(PP, L), sm, st>>>(ma);                                 \
   }
+#define CALL_MF(PP)                                                                       \
+  if (narrow((d.xc + lines_for(PP) - 1) / lines_for(PP) * 3 * d.nz)) CALL_MF_L(PP, lines_narrow(PP)) else CALL_MF_L(PP, lines_for(PP))
     if (mmx_mid_col_ok(d.py, d.ny)) {
       if (int rc = mmx_mid_col_launch(w, d.py, -1, d.spec1, d.spec2, d.ny, d.py, ma.in_outer, ma.out_outer,
                                       3 * d.nz, d.tw[1])) return rc;
@@ -366,15 +378,16 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
       ia.odd_inner = (1u << 3) | (1u << 5); ia.odd_outer = 0;
       ia.two_d = 1; ia.tw = d.tw[1];
     }
-#define CALL_IN(PP)                                                                       \
+#define CALL_IN_L(PP, L)                                                                  \
   {                                                                                       \
-    constexpr int L = lines_for(PP);                                                      \
     size_t sm = sizeof(float2) * 3 * PP * L;                                              \
-    if (int rc = set_smem(k_inner<PP>, sm)) return rc;                                    \
+    if (int rc = set_smem(k_inner<PP, L>, sm)) return rc;                                 \
     dim3 g((d.xc + L - 1) / L, nouter);                                                   \
     ProfScope ps(w, PK_INNER);                                                             \
-    k_inner<PP><<<g, block_for(PP), sm, st>>>(ia);                                        \
+    k_inner<PP, L><<<g, block_of(PP, L), sm, st>>>(ia);                                   \
   }
+#define CALL_IN(PP)                                                                       \
+  if (narrow((d.xc + lines_for(PP) - 1) / lines_for(PP) * nouter)) CALL_IN_L(PP, lines_narrow(PP)) else CALL_IN_L(PP, lines_for(PP))
     if (d.tiled) {
       if (int rc = mmx_inner_tile_launch(w)) return rc;
     } else if (mmx_inner_col_ok(d, Pin, ia.n_valid)) {
@@ -395,15 +408,16 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     ma.n_in = d.py; ma.n_out = d.ny; ma.xc = d.xc; ma.xp = d.xp; ma.gated = 1;
     ma.in_outer = (size_t)d.py * d.xp; ma.out_outer = (size_t)d.ny * d.xp;
     ma.in = d.spec2; ma.out = d.spec1; ma.tw = d.tw[1]; ma.ctrl = w->d_ctrl;
-#define CALL_MI(PP)                                                                       \
+#define CALL_MI_L(PP, L)                                                                  \
   {                                                                                       \
-    constexpr int L = lines_for(PP);                                                      \
     size_t sm = sizeof(float2) * PP * L;                                                  \
-    if (int rc = set_smem(k_mid<PP, +1>, sm)) return rc;                                  \
+    if (int rc = set_smem(k_mid<PP, L, +1>, sm)) return rc;                               \
     dim3 g((d.xc + L - 1) / L, 3 * d.nz);                                                 \
     ProfScope ps(w, PK_MID_INV);                                                           \
-    k_mid<PP, +1><<<g, block_for(PP), sm, st>>>(ma);                                      \
+    k_mid<PP, L, +1><<<g, block_of(PP, L), sm, st>>>(ma);                                 \
   }
+#define CALL_MI(PP)                                                                       \
+  if (narrow((d.xc + lines_for(PP) - 1) / lines_for(PP) * 3 * d.nz)) CALL_MI_L(PP, lines_narrow(PP)) else CALL_MI_L(PP, lines_for(PP))
     if (mmx_mid_col_ok(d.py, d.ny)) {
       if (int rc = mmx_mid_col_launch(w, d.py, +1, d.spec2, d.spec1, d.py, d.ny, ma.in_outer, ma.out_outer,
                                       3 * d.nz, d.tw[1])) return rc;
@@ -413,14 +427,15 @@ int mmx_demag_launch(mmx_world* w, const float* const yin[2], float* bout) {
     w->launches++;
   }
 
-#define CALL_XI(PP)                                                                       \
+#define CALL_XI_L(PP, L)                                                                  \
   {                                                                                       \
-    constexpr int L = lines_for(PP);                                                      \
     size_t sm = sizeof(float2) * PP * (L | 1);                                            \
-    if (int rc = set_smem(k_x_inv<PP>, sm)) return rc;                                    \
+    if (int rc = set_smem(k_x_inv<PP, L>, sm)) return rc;                                 \
     ProfScope ps(w, PK_X_INV);                                                             \
-    k_x_inv<PP><<<(rows + 2 * L - 1) / (2 * L), block_for(PP), sm, st>>>(xa);             \
+    k_x_inv<PP, L><<<(rows + 2 * L - 1) / (2 * L), block_of(PP, L), sm, st>>>(xa);        \
   }
+#define CALL_XI(PP)                                                                       \
+  if (narrow_rows((rows + 2 * lines_for(PP) - 1) / (2 * lines_for(PP)))) CALL_XI_L(PP, lines_narrow(PP)) else CALL_XI_L(PP, lines_for(PP))
   if (xwarp) {
     if (int rc = mmx_x_warp_launch(w, +1, yin, bout)) return rc;
   } else {
