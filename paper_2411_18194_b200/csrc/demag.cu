@@ -85,19 +85,15 @@ __global__ void __launch_bounds__(block_of(P, L)) k_x_fwd(XArgs a) {
   const float* y = a.yin[a.ctrl->sel];
   const int tid = threadIdx.x, T = L * TPL;
   const long long row0 = (long long)blockIdx.x * (2 * L);
+  const unsigned rpc = (unsigned)a.rows / 3u;   // rows per component: the cell of element (row r, x) is (r mod rpc) nx + x
+#pragma unroll
   for (int idx = tid; idx < L * P; idx += T) {
     const int line = idx / P, x = idx % P;
     float2 v = make_float2(0.f, 0.f);
     if (x < a.nx) {
-      const long long r0 = row0 + 2 * line;
-      if (r0 < a.rows) {
-        size_t off = (size_t)r0 * a.nx + x;
-        v.x = gather_M(a, y, off, off % a.N);
-      }
-      if (r0 + 1 < a.rows) {
-        size_t off = (size_t)(r0 + 1) * a.nx + x;
-        v.y = gather_M(a, y, off, off % a.N);
-      }
+      const unsigned r0 = (unsigned)row0 + 2u * (unsigned)line;   // (32-bit index arithmetic: rows < 2^31)
+      if (r0 < (unsigned)a.rows) v.x = gather_M(a, y, (size_t)r0 * a.nx + x, (size_t)(r0 % rpc) * a.nx + x);
+      if (r0 + 1 < (unsigned)a.rows) v.y = gather_M(a, y, (size_t)(r0 + 1) * a.nx + x, (size_t)((r0 + 1) % rpc) * a.nx + x);
     }
     s[x * LP + line] = v;
   }
