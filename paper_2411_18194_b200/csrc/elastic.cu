@@ -47,9 +47,11 @@ __device__ __forceinline__ float grad1(const float* f, int i, int n, bool per, s
 }
 
 __device__ __forceinline__ void coords(size_t i, const int n[3], int p[3]) {
-  p[0] = (int)(i % n[0]);
-  p[1] = (int)((i / n[0]) % n[1]);
-  p[2] = (int)(i / ((size_t)n[0] * n[1]));
+  // (32-bit arithmetic: a world has fewer than 2^31 cells, mmx_world_create checks it)
+  const unsigned c = (unsigned)i, row = c / (unsigned)n[0];
+  p[0] = (int)(c - row * (unsigned)n[0]);
+  p[2] = (int)(row / (unsigned)n[1]);
+  p[1] = (int)(row - (unsigned)p[2] * (unsigned)n[1]);
 }
 
 __global__ void __launch_bounds__(256) k_strain(ElasticArgs a) {
@@ -142,7 +144,8 @@ __global__ void __launch_bounds__(256) k_elastic(ElasticArgs a) {
   const float* yin = a.yin[sel];
   // traction amplitude at the stage time
   float tr[3] = {0.f, 0.f, 0.f};
-  if (a.face >= 0) {
+  // (only the cells on the traction face use it: the fp64 sine is not evaluated by the others)
+  if (a.face >= 0 && p[a.face >> 1] == ((a.face & 1) ? n[a.face >> 1] - 1 : 0)) {
     double t = a.t_fixed;
     if (a.ctrl && !a.accel_out) t = a.ctrl->t + (double)a.ctrl->cc[a.stage] * a.ctrl->dt;
     const double amp = a.tamp * sin(2.0 * 3.14159265358979323846 * a.tfreq * t);

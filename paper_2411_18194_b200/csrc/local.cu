@@ -129,7 +129,9 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
   float errv = 0.f, tqv = 0.f;
   bool bad = false;
   if (i < N) {
-    const int ix = (int)(i % a.nx), iy = (int)((i / a.nx) % a.ny), iz = (int)(i / ((size_t)a.nx * a.ny));
+    // (32-bit index arithmetic: a world has fewer than 2^31 cells)
+    const unsigned ci = (unsigned)i, rowi = ci / (unsigned)a.nx;
+    const int ix = (int)(ci - rowi * (unsigned)a.nx), iz = (int)(rowi / (unsigned)a.ny), iy = (int)(rowi - (unsigned)iz * (unsigned)a.ny);
     const int rc = REG ? a.reg[i] : 0;
     long long ni[6];
     int rn[6];
@@ -176,11 +178,12 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a) {
               mn = mnb[s][q];
               const bool same = rn[q] == rc;
               if (a.terms & MMX_T_EXCH) {
-                const float wex = 2.f * harm(Ac, Pn[MP_A]) * (same ? 1.f : a.scaleA11) * iMs * a.inv_h2[axis];
+                // (same region: the harmonic mean of A with itself is A -- no division)
+                const float wex = 2.f * (same ? Ac : harm(Ac, Pn[MP_A]) * a.scaleA11) * iMs * a.inv_h2[axis];
                 B = fma3(wex, mn - mc[s], B);
               }
               if (axis < 2 && (a.terms & MMX_T_DMI)) {
-                const float wd = harm(Dc, Pn[MP_D]) * iMs * a.inv_h[axis] * d;
+                const float wd = (same ? Dc : harm(Dc, Pn[MP_D])) * iMs * a.inv_h[axis] * d;
                 // (z x (d e_axis)) x m_n = d (m_z e_axis - m_axis z)
                 if (axis == 0) { B.x = fmaf(wd, mn.z, B.x); B.z = fmaf(-wd, mn.x, B.z); }
                 else { B.y = fmaf(wd, mn.z, B.y); B.z = fmaf(-wd, mn.y, B.z); }
