@@ -37,9 +37,17 @@ constexpr int NW = 8;                              // warps per CTA, two columns
 constexpr int XS_BYTES = 3 * H * TL * 8;           // one spectrum stage: 24576
 constexpr int KS_FLOATS = 6 * (H + 1) * TL;        // one kernel image: 6240 floats
 constexpr int KS_BYTES = KS_FLOATS * 4;            // 24960
-constexpr int EXR = 2 * (H + 8) * 2;               // float2 per exchange region: [half][72 padded rows][2 columns]
-constexpr int EX_BYTES = NW * 2 * EXR * 8;         // two regions per warp: 36864
-constexpr int SMEM_BYTES = 2 * XS_BYTES + KS_BYTES + EX_BYTES + 64;
+// Measured on c4: 2 stages + 2 regions 135.5 us; 2 + 1 (the components serialise on the one region) 140.5 us;
+// 3 stages + 1 region (what fits beside the kernel image at two CTAs per SM) 139.4 us
+constexpr int NXS = 2;                             // spectrum stages
+constexpr int NEXR = 2;                            // exchange regions per warp
+constexpr int EXR = 2 * H * 2;                     // float2 per exchange region: [half][64 rows, XOR-swizzled][2 columns]
+constexpr int EX_BYTES = NW * NEXR * EXR * 8;
+constexpr int SMEM_BYTES = NXS * XS_BYTES + KS_BYTES + EX_BYTES + 64;
+// row (q, j) of an exchange region: q 8 + (j ^ q).  The radix-8 stage of thread j writes rows (q, j) and reads rows (j, q)
+// (or the other way round): both are conflict-free, the first because the eight lanes j fill one 128-byte group, the
+// second because row (j, q) sits at offset (q ^ j) of group j
+__device__ __forceinline__ int exrow(int q, int j) { return (q * 8 + (j ^ q)) * 2; }
 
 struct TileArgs {
   float2* spec;          // spec2 in tile-major layout
@@ -117,12 +125,12 @@ __device__ __forceinline__ TilePos tile_pos(const TileArgs& a, int T) {
 __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
   extern __shared__ __align__(128) unsigned char smraw[];
   float2* xs0 = reinterpret_cast<float2*>(smraw);
-  float* ks = reinterpret_cast<float*>(smraw + 2 * XS_BYTES);
-  float2* exw = reinterpret_cast<float2*>(smraw + 2 * XS_BYTES + KS_BYTES);
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smraw + 2 * XS_BYTES + KS_BYTES + EX_BYTES);
-  unsigned long long* full = bars;       // [2] "spectrum stage s has landed"
-  unsigned long long* kfull = bars + 2;  // "kernel image has landed"
-  int* cnt = reinterpret_cast<int*>(bars + 3);  // [2] tickets "warps done with stage s", [2] "warps past the multiply"
+  float* ks = reinterpret_cast<float*>(smraw + NXS * XS_BYTES);
+  float2* exw = reinterpret_cast<float2*>(smraw + NXS * XS_BYTES + KS_BYTES);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smraw + NXS * XS_BYTES + KS_BYTES + EX_BYTES);
+  unsigned long long* full = bars;       // [NXS] "spectrum stage s has landed"
+  unsigned long long* kfull = bars + 3;  // "kernel image has landed"
+  int* cnt = reinterpret_cast<int*>(bars + 4);  // [NXS] tickets "warps done with stage s", [3] "warps past the multiply"
 
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int col = lane & 1, j = (lane >> 1) & 7, h = lane >> 4;
@@ -139,6 +147,7 @@ __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
   const int G = gridDim.x;
   const unsigned xbytes = (unsigned)a.nz * TL * 8;  // one component of a tile
   auto seqT = [&](int i) -> int { return 2 * ((int)blockIdx.x + G * (i >> 1)) + (i & 1); };
+  static_assert(NXS == 2 || NXS == 3, "two or three spectrum stages");
   auto load_tile = [&](int T, int s) {
     const TilePos p = tile_pos(a, T);
     mbar_expect_tx(&full[s], 3 * xbytes);
@@ -153,33 +162,36 @@ __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
   };
 
   if (a.nz < H) {  // rows that are zero padding: cleared once, never written (generic proxy, fenced below)
-    for (int q = threadIdx.x; q < 2 * XS_BYTES / 16; q += 32 * NW) reinterpret_cast<float4*>(smraw)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int q = threadIdx.x; q < NXS * XS_BYTES / 16; q += 32 * NW) reinterpret_cast<float4*>(smraw)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   if (threadIdx.x == 0) {
-    mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_init(kfull, 1);
-    cnt[0] = cnt[1] = cnt[2] = cnt[3] = 0;
+    for (int q = 0; q < NXS; ++q) mbar_init(&full[q], 1);
+    mbar_init(kfull, 1);
+    for (int q = 0; q < 6; ++q) cnt[q] = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
   if (threadIdx.x == 0 && seqT(0) < a.ntiles) {
     load_tile(seqT(0), 0);
     load_kimg(tile_pos(a, seqT(0)).img);
-    if (seqT(1) < a.ntiles) load_tile(seqT(1), 1);
+    for (int q = 1; q < NXS; ++q)
+      if (seqT(q) < a.ntiles) load_tile(seqT(q), q);
   }
 
   // per-thread constants of the swizzled layouts
   const int pos_lo = ((w ^ j) << 1) | col;                    // spectrum rows z with (z & 7) = j; kernel rows kz <= 64
   const int pos_hi = ((w ^ ((-j - h) & 7)) << 1) | col;       // mirrored kernel rows 128 - kz
-  float2* ex0 = exw + w * 2 * EXR + h * ((H + 8) * 2) + col;  // this thread's half of region 0
+  float2* ex0 = exw + w * NEXR * EXR + h * (H * 2) + col;      // this thread's half of region 0
   const float* kp_lo = ks + (2 * j + h) * TL + pos_lo;
   const float* kp_hi = ks + (P - 2 * j - h) * TL + pos_hi;
   const unsigned mi3 = ((a.odd_inner >> 3) & 1u) << 31, mi4 = ((a.odd_inner >> 4) & 1u) << 31, mi5 = ((a.odd_inner >> 5) & 1u) << 31;
 
   unsigned kuse = 0, prev_img = 0xffffffffu;
   int T = seqT(0);
+  int s = 0;
+  unsigned par = 0;   // parity of the current use of stage s
   for (int i = 0; T < a.ntiles; ++i) {
-    const int s = i & 1;
     const TilePos tp = tile_pos(a, T);
     const int Tn = seqT(i + 1);
     const bool more = Tn < a.ntiles;
@@ -188,21 +200,21 @@ __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
     const int ky = tp.nyq ? tp.ky + 2 * w + col : tp.ky;
     const unsigned so = 2 * ky > a.py ? 1u : 0u;
 
-    mbar_wait(&full[s], (unsigned)(i >> 1) & 1u);
+    mbar_wait(&full[s], par);
     float2 X[3][R];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
 #pragma unroll
       for (int u = 0; u < R; ++u) X[c][u] = cmul(xs[(c * H + j + R * u) * TL], twp[u]);
       Dft<R, -1>::run(X[c]);
-      float2* t = ex0 + (c & 1) * EXR;
-      if (c == 2) __syncwarp();  // region 0 is reused: component 0 has been read by every lane
-      t[(0 * 9 + j) * 2] = X[c][0];
+      float2* t = ex0 + (c % NEXR) * EXR;
+      if (c >= NEXR) __syncwarp();  // the region is reused: its previous component has been read by every lane
+      t[exrow(0, j)] = X[c][0];
 #pragma unroll
-      for (int q = 1; q < R; ++q) t[(q * 9 + j) * 2] = cmul(X[c][q], tws[q]);
+      for (int q = 1; q < R; ++q) t[exrow(q, j)] = cmul(X[c][q], tws[q]);
       __syncwarp();
 #pragma unroll
-      for (int q = 0; q < R; ++q) X[c][q] = t[(j * 9 + q) * 2];
+      for (int q = 0; q < R; ++q) X[c][q] = t[exrow(j, q)];
       Dft<R, -1>::run(X[c]);
     }
     if (tp.img != prev_img) {  // a new kernel image was requested for this tile
@@ -230,8 +242,8 @@ __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
       __syncwarp();
       if (lane == 0) {
         __threadfence_block();
-        if (atomicAdd(&cnt[2], 1) == NW - 1) {
-          cnt[2] = 0;
+        if (atomicAdd(&cnt[NXS], 1) == NW - 1) {
+          cnt[NXS] = 0;
           __threadfence_block();
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           load_kimg(next_img);
@@ -241,14 +253,14 @@ __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
       Dft<R, +1>::run(X[c]);
-      float2* t = ex0 + (c & 1) * EXR;
+      float2* t = ex0 + (c % NEXR) * EXR;
       __syncwarp();  // the region's previous contents have been read by every lane
-      t[(j * 9 + 0) * 2] = X[c][0];
+      t[exrow(j, 0)] = X[c][0];
 #pragma unroll
-      for (int q = 1; q < R; ++q) t[(j * 9 + q) * 2] = cmulc(X[c][q], tws[q]);
+      for (int q = 1; q < R; ++q) t[exrow(j, q)] = cmulc(X[c][q], tws[q]);
       __syncwarp();
 #pragma unroll
-      for (int q = 0; q < R; ++q) X[c][q] = t[(q * 9 + j) * 2];
+      for (int q = 0; q < R; ++q) X[c][q] = t[exrow(q, j)];
       Dft<R, +1>::run(X[c]);
 #pragma unroll
       for (int b = 0; b < R; ++b) X[c][b] = cmulc(X[c][b], twp[b]);
@@ -279,7 +291,7 @@ __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
           bulk_s2g(a.spec + tp.off + (unsigned)c * (unsigned)(a.nz * TL),
                    reinterpret_cast<unsigned char*>(xs0) + s * XS_BYTES + c * (H * TL * 8), xbytes);
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        const int T2 = seqT(i + 2);
+        const int T2 = seqT(i + NXS);
         if (T2 < a.ntiles) {
           asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // the stage has been read out
           load_tile(T2, s);
@@ -287,6 +299,7 @@ __global__ void __launch_bounds__(32 * NW, 2) k_inner_tile(TileArgs a) {
       }
     }
     T = Tn;
+    if (++s == NXS) { s = 0; par ^= 1u; }
   }
   if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // my write-backs are complete
 }
