@@ -176,6 +176,11 @@ def test_elastic_3d_and_periodic():
 # kernel) only engage on grids shaped like c4; these cases are the smallest ones that reach every
 # variant: mid pass R = 4 (Py = 32), R = 8 (Py = 128), R = 16 (Py = 512), inner pass P = 128.
 FAST_CASES = [(132, 12, 40), (136, 40, 36), (256, 130, 33), (192, 64, 64)]
+# Shapes that take the tile-major inner pass (demag_tile.cu: Pz = 128, Py = 512, enough tiles for the pipelined y pass)
+# with other tile counts than c4's: Px = 256 (8 column tiles per ky, warp x passes do not apply), Px = 1024 (32 column
+# tiles, generic x passes), fewer z rows than 64 (zero-padded stage rows), three regions with an empty one (generic x
+# passes with the per-cell Ms gather in front of the tiled passes).
+TILED_CASES = [((128, 130, 60), False), ((260, 130, 34), False), ((256, 136, 40), True)]
 
 
 @pytest.mark.parametrize("grid", FAST_CASES)
@@ -191,6 +196,25 @@ def test_fast_path_fields(grid):
     assert e < FIELD_TOL, (grid, "total", e)
     e = field_err(g.eval_torque(0), o.torque(0))
     assert e < FIELD_TOL, (grid, "torque", e)
+    g.destroy()
+
+
+@pytest.mark.parametrize("grid,regions", TILED_CASES)
+def test_tile_major_inner_pass_other_shapes(grid, regions):
+    spec = wl.make("c4", grid)
+    rng = np.random.default_rng(91)
+    if regions:
+        spec.regions = rng.integers(0, 3, (grid[2], grid[1], grid[0])).astype(np.uint16)
+        spec.mat = wl.make_mat(1, 3, Ms=np.array([[1.0e6, 0.0, 6.0e5]]), A=np.array([[1.0e-11, 1.0e-11, 0.7e-11]]), alpha=0.1)
+    g, o = pair(spec)
+    magnetic = (o.p[0]["Ms"] > 0)[None]
+    for bit in (mmx.T_DEMAG, mmx.T_ALL):
+        e = field_err(g.eval_heff(0, bit), o.heff(0, terms=bit) * magnetic)
+        assert e < FIELD_TOL, (grid, bit, e)
+    st = g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=1e-13, nsteps=3)
+    o.step_dp45_fixed(1e-13, 3)
+    assert st["accepted"] == 3
+    assert np.abs(g.get_state(mmx.F_M0).astype(np.float64) - o.m[0]).max() <= 1e-4
     g.destroy()
 
 
