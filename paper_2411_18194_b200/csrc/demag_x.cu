@@ -139,15 +139,16 @@ __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   }
 }
 
-struct __align__(16) XInvSmem {
-  float2 in[2][XH + 4];      // [row a / b][257 kept columns, padded to 16 B]
+struct __align__(128) XInvSmem {
+  float2 in[2][XH + 16];     // [row a / b][257 kept columns]; rows and the struct are multiples of 128 bytes, so a warp's
+                             // 512-byte cp.async lands on four bank rows, not five (10 % of this pass's wavefronts)
   float2 ex[2 * EXN];         // exchange tiles; reused as the two output rows [2][256] floats
 };
 
 template <bool FULL>
 __global__ void __launch_bounds__(32 * XW, 3) k_x_inv_w(XWArgs a) {
   const int nx = FULL ? XH : a.nx;
-  extern __shared__ __align__(16) unsigned char smraw[];
+  extern __shared__ __align__(128) unsigned char smraw[];
   __shared__ float2 stw[XH];  // conj(w_P^n) for the first P/2 outputs only
   // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
   // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
