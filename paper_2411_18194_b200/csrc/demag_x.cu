@@ -54,7 +54,7 @@ __host__ __device__ inline size_t xfwd_warp_bytes(int S) { return (size_t)S * 2 
 template <bool FULL>
 __global__ void __launch_bounds__(32 * XW, 4) k_x_fwd_w(XWArgs a) {
   const int nx = FULL ? XH : a.nx, S = FULL ? 1 : a.S;
-  extern __shared__ __align__(16) unsigned char smraw[];
+  extern __shared__ __align__(128) unsigned char smraw[];
   __shared__ float2 stw[XH];  // w_P^n for n < P/2 only (the half twiddles of the pruned input)
   // stage twiddles w_H^(j q) laid out [j][q] with a row pitch of 17: lanes (different j, same q) hit
   // different banks (stw[2 j q] has a lane stride of 4 q words: up to 8-way conflicts)
