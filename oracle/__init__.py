@@ -20,7 +20,14 @@ Pin status (see tests/test_oracle_*.py and DESIGN.md section "Oracle pins"):
                             embedded pairs of Table 2, observed orders, estimate scaling)
   Zhang-Li torque ......... pinned (P13: Gilbert-form identity, rigid translation at -u)
   elastic / magnetoelastic  pinned (P15 paper numbers, P16 patch test, P17; viscous term P20 paper numbers)
-  adaptive-step controller constants (S21), PBC image window (S13), which
-  config switches c3 uses (S8, S14): parity unpinned -- definitions shared by
-  both sides, stated in DESIGN.md.
+  inter-sublattice DMI tensor pinned (P22b); three sublattices pinned (P25: pair-energy gradients, 120-degree state)
+  Slonczewski torque ...... pinned (P23: macrospin closed form, switching current, eps at three angles; reading S37)
+  relaxation mode ......... pinned (P24: closed form without precession, energy descent); the path it takes: unpinned
+  stray field at height ... pinned (P26: on-axis closed form, dipole limit, tie to the in-magnet kernel; reading S40)
+  Neumann boundary (Eq.5) . pinned (P27: Eq.5 as printed, collinear-AFM closed form, exact 1/h cancellation); which of the
+                            two continuum-equivalent discretisations (open S9 / ghost cells S41) mumax+ shows at finite
+                            cell size: parity unpinned
+  adaptive-step controller constants (S21), PBC image window (S13), which config switches c3 uses (S8, S14), Zhang-Li
+  with two sublattices (S18), the error norm with (u, v) (S22), the DMI chirality sign (S7), the cell-averaged probe of
+  S40: parity unpinned -- definitions shared by both sides, stated in DESIGN.md.
 """
