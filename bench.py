@@ -429,6 +429,29 @@ def run_mmx(args, rank, local_rank, world_size):
                              "cell_updates_per_s": ospec.ncells * 1e3 / oms,
                              "frac_of_8TBs_survey_model": survey_step_bytes(ospec) / (oms * 1e-3) / 8e12}
             og.destroy()
+            # a parameter sweep (the paper's demo 2.1 sweeps current and exchange reduction): independent worlds of
+            # the same recipe, one stream and one host thread each; aggregate throughput over all of them
+            import threading
+            nw = 8
+            ws = []
+            for k in range(nw):
+                stk = torch.cuda.Stream()
+                ws.append((mmx.World.from_spec(wl.make(oname, seed=2000 + k), stream=stk.cuda_stream), stk))
+            stepk = lambda gw, n: gw.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=DT[oname], nsteps=n)
+            for gw, _ in ws:
+                stepk(gw, 5)
+            torch.cuda.synchronize()
+            tw0 = time.perf_counter()
+            th = [threading.Thread(target=stepk, args=(gw, ko)) for gw, _ in ws]
+            for t_ in th:
+                t_.start()
+            for t_ in th:
+                t_.join()
+            torch.cuda.synchronize()
+            tw = time.perf_counter() - tw0
+            others[oname]["sweep_of_8_worlds_cell_updates_per_s"] = nw * ospec.ncells * ko / tw
+            for gw, _ in ws:
+                gw.destroy()
 
     cpu = None
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
