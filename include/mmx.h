@@ -273,6 +273,52 @@ int mmx_max_torque(mmx_world* w, double* out);
  * out: fp32 [3][Ny][Nx] tesla, host or device.  A direct sum: meant for imaging a state, not for the time loop. */
 int mmx_stray_field(mmx_world* w, double height, float* out, int mem);
 
+/* The same probe-layer field (Fig.3; P:L144 for M = sum_s Ms m_s; reading S40) for callers that may not allocate.
+ *
+ * mmx_stray_field cudaMallocs and cudaFrees its Newell table on every call and needs a world, which owns cudaMalloc'd
+ * storage of its own.  Some callers cannot afford either: a process whose device memory is held in full by a pooling
+ * allocator (PyTorch / CuPy caching allocator, a serving arena), where a raw cudaMalloc fails or forces the pool to be
+ * flushed; a latency-bound loop, because cudaMalloc / cudaFree take a driver-wide lock and cudaFree waits for the device;
+ * a thread that runs while another thread captures a CUDA graph in the global capture mode, which a cudaMalloc breaks.
+ * mmx_stray_field_static is the entry point for them.  It needs no world.  It calls no cudaMalloc, cudaFree,
+ * cudaMallocAsync or other allocating routine and uses no host heap; its only scratch memory, M = sum_s Ms m_s as
+ * [3][Nz][Ny][Nx] fp32, lives in an array built into the library's CUDA module.
+ *
+ *   limit     Nx*Ny*Nz <= MMX_STRAY_STATIC_MAX_CELLS (262 144, e.g. 512 x 512 x 1; the paper's Fig.3 film is
+ *             500 x 500 x 1).  Larger grids: MMX_EINVAL with a message that names the limit, nothing is launched.
+ *   cost      12 * MMX_STRAY_STATIC_MAX_CELLS bytes = 3 MiB of device memory on every GPU on which the library's CUDA
+ *             module gets loaded, from that moment until the process exits, whether or not this call is ever made.
+ *   grid      (Nx, Ny, Nz), host.   n_sublattices 1..3.   Ms[n_sublattices] host, A/m, one value per sublattice (the
+ *             magnet is uniform here: no region map; an empty cell is m = 0 in that cell).
+ *   m         DEVICE, fp32 [n_sublattices][3][Nz][Ny][Nx], the reduced magnetisations.   Caller-owned, read only.
+ *   table     DEVICE, fp32 [Nz][6][Ny][Nx]: the z-shifted Newell tensor per source layer with -mu0 folded in, exactly the
+ *             numbers mmx_stray_table_host writes (build it once per grid / cell size / height, copy it into device
+ *             memory you already own).  Caller-owned, read only.
+ *   out       DEVICE, fp32 [3][Ny][Nx], tesla.  Caller-owned; every element is written.
+ *   cuda_stream  cudaStream_t as void*; NULL = the legacy default stream.  Two kernels are enqueued on it and the call
+ *             returns without waiting for them (read `out` in stream order, or after synchronising the stream).
+ * All pointers must belong to the device that is current when the call is made.
+ *
+ * First call on a device.  The first call made with a given device current also does a one-time set-up for that device:
+ * it asks the runtime for the device address of the built-in array (cudaGetSymbolAddress; this is also what makes the
+ * runtime load the module there).  Make that first call -- one per device you use -- before any stream capture is started.
+ *
+ * Sharing.  Every call on a device uses the same array, and the array keeps what the previous call left in it.  Nothing
+ * in it has to start at zero: a call overwrites elements [0, 3 Nx Ny Nz) before it reads them, in stream order.  Calls
+ * that overlap in time on one GPU (different streams, several host threads, several worlds) race on the array and return
+ * garbage without any error: order them on one stream, or with events.  Calls on different GPUs do not interact.
+ *
+ * Errors: MMX_EINVAL (NULL pointer, sizes, the limit above, a device ordinal >= 64), MMX_ECUDA (set-up or launch failed).
+ * Pointers are not checked for being device pointers. */
+#define MMX_STRAY_STATIC_MAX_CELLS 262144
+int mmx_stray_field_static(const int grid[3], int n_sublattices, const double Ms[], const float* m, const float* table,
+                           float* out, void* cuda_stream);
+/* Host-only helper, needs no GPU: the table mmx_stray_field_static takes, fp32 [Nz][6][Ny][Nx] (components xx, yy, zz, xy,
+ * xz, yz on the non-negative quadrant of in-plane offsets; layer k at z offset (Nz - k - 1/2) dz + height; times -mu0),
+ * the same values mmx_stray_field builds internally.  out_len must be Nz*6*Ny*Nx.  Ordinary host code: it uses the host
+ * heap and may take seconds on large grids; run it once, at set-up. */
+int mmx_stray_table_host(const int grid[3], const double cellsize[3], double height, float* out, long long out_len);
+
 /* ---- time stepping --------------------------------------------------------------------- */
 
 /* nsteps classical RK4 steps of size dt (BASELINE config 1 protocol). */

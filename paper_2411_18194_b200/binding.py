@@ -105,6 +105,8 @@ PROTOTYPES = {
     "mmx_step_rk4": (C.c_int, [_W, C.c_double, C.c_longlong]),
     "mmx_step_rk45": (C.c_int, [_W, C.POINTER(RkOpts), C.POINTER(RkStats)]),
     "mmx_stray_field": (C.c_int, [_W, C.c_double, C.c_void_p, C.c_int]),
+    "mmx_stray_field_static": (C.c_int, [_I3, C.c_int, _D3, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "mmx_stray_table_host": (C.c_int, [_I3, _D3, C.c_double, C.c_void_p, C.c_longlong]),
     "mmx_relax": (C.c_int, [_W, C.c_double, C.c_double, C.c_longlong, C.POINTER(RkStats)]),
     "mmx_get_err_history": (C.c_int, [_W, _D3, C.c_int, _I3]),
     "mmx_profile_enable": (C.c_int, [_W, C.c_int]),
@@ -176,6 +178,29 @@ def kernel_spectrum_host(grid, cell, pbc=(0, 0, 0), cutoff_cells=32.0):
     out = np.empty((6, kz, ky, xp), dtype=np.float32)
     _check(lib.mmx_kernel_spectrum_host(*a, float(cutoff_cells), out.ctypes.data, out.size, dims))
     return out, (px, py, pz)
+
+
+STRAY_STATIC_MAX_CELLS = 262144
+
+
+def stray_table_host(grid, cell, height) -> np.ndarray:
+    """mmx_stray_table_host: fp32 [Nz][6][Ny][Nx], the table mmx_stray_field_static takes; needs no GPU."""
+    out = np.empty((grid[2], 6, grid[1], grid[0]), dtype=np.float32)
+    _check(load().mmx_stray_table_host(_arr(C.c_int, list(grid)), _arr(C.c_double, list(cell)), float(height),
+                                       out.ctypes.data, out.size))
+    return out
+
+
+def stray_field_static(grid, Ms, m, table, out, stream=None):
+    """mmx_stray_field_static: the probe-layer field without any allocation inside the library (see include/mmx.h for
+    who needs that, the cell limit and the sharing rules).  m [S][3][Nz][Ny][Nx], table [Nz][6][Ny][Nx] and
+    out [3][Ny][Nx] are contiguous fp32 CUDA tensors the caller owns; Ms has one value per sublattice.  The result is in
+    `out` in stream order; nothing is returned and nothing is synchronised."""
+    for t in (m, table, out):
+        assert t.is_cuda and t.is_contiguous() and t.element_size() == 4
+    Ms = [float(v) for v in Ms]
+    _check(load().mmx_stray_field_static(_arr(C.c_int, list(grid)), len(Ms), _arr(C.c_double, Ms), m.data_ptr(),
+                                         table.data_ptr(), out.data_ptr(), C.c_void_p(stream) if stream else None))
 
 
 class World:

@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmmx.so")
 BUILD = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "local.cu", "demag.cu", "demag_col.cu", "demag_tile.cu", "demag_x.cu", "elastic.cu", "stray.cu", "newell.cpp"]
+SOURCES = ["api.cu", "local.cu", "demag.cu", "demag_col.cu", "demag_tile.cu", "demag_x.cu", "elastic.cu", "stray.cu", "stray_static.cu", "newell.cpp"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC,-fopenmp,-O2", "-I", os.path.join(ROOT, "include")]
