@@ -13,7 +13,8 @@ Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline /
 
 Pin status (see tests/test_oracle_*.py and DESIGN.md section "Oracle pins"):
   newell / demag .......... pinned (P1-P5, P19, mpmath spot values, dipole limit)
-  exchange, DMI, anisotropy pinned (P6, P10, P11; general DMI tensor of Eq.4: P22)
+  exchange, DMI, anisotropy pinned (P6, P10, P11; general DMI tensor of Eq.4: P22; uniaxial: P12; cubic: P28 textbook energy
+                            values along <100>, <110>, <111> and the precession frequency gamma 2 Kc1/Ms about an easy axis)
   sublattice exchange ..... pinned (A12 term: P6b two-sublattice spin waves, factor and partner wiring;
                             A0 term: P12); homogeneous DMI Eq.6 pinned (P21)
   LLG torque, integrators . pinned (P7, P8, P9; P14: rooted-tree order conditions of RK4 and of all five

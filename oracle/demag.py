@@ -7,7 +7,7 @@ Definition:  B_i(r) = -mu0 sum_{r'} sum_j K_ij(r - r') M_j(r'
 M = sum_s Ms^(s) m^(s).  `demag_direct` IS that definition (O(N^2));
 `demag_fft` is the same convolution through zero-padded FFTs (scipy.fft as a
 library step) and is validated against the direct sum in
-tests/test_oracle_demag.py (P5).
+tests/test_oracle_newell.py (P5).
 """
 from __future__ import annotations
 

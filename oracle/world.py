@@ -109,7 +109,11 @@ class World:
         # first two" -- reading S38: the terms are summed over both partners)
         others = [t for t in range(self.S) if t != s]
         out = {}
-        gh = self.ghosts(m) if self.cpl.get("bc") == "neumann" else None   # Eq.5 (reading S41); None: open / periodic
+        # P:L161 "The Neumann boundary conditions as given in Eq. (5) are the default in mumax+.  Alternatively, open or
+        # periodic boundary conditions can be used": Eq.5 unless the world asks for "open"; three sublattices are open
+        # (Eq.5 is written for a sublattice and its partner, reading S41)
+        bc = self.cpl.get("bc") or ("neumann" if self.S <= 2 else "open")
+        gh = self.ghosts(m) if bc == "neumann" else None   # Eq.5 (reading S41); None: open
         G = (lambda t: None) if gh is None else (lambda t: gh[t])
         if terms & T_EXCH:
             out[T_EXCH] = fl.pair_laplacian(m[s], p["Ms"], p["A"], self.reg, self.cpl["scale_A11"],

@@ -146,7 +146,7 @@ def _small_world(alpha, seed=21, S=1, J=(0, 0, 0)):
     spec = wl.WorldSpec(
         name="small", grid=grid, cell=(3e-9, 3e-9, 2e-9), S=S,
         mat=wl.make_mat(S, Ms=8e5, A=1.3e-11, alpha=alpha, Ku1=5e4, D=1e-3, Kc1=2e4),
-        coupling=wl.default_coupling(A0=-4e-15, A12=-1e-12, D_inter=3e-4), bext=(0.0, 0.01, 0.05), J=J,
+        coupling=wl.default_coupling(A0=-4e-15, A12=-1e-12, D_inter=3e-4, bc="open"), bext=(0.0, 0.01, 0.05), J=J,   # open: the BC of the pair energy
         m=[wl.smoothed_random_unit(rng, grid, 2.0) for _ in range(S)])
     return World(spec, demag_mode="direct")
 
@@ -364,3 +364,61 @@ def test_P24_relaxation_closed_form_and_energy_descent():
     assert st["accepted"] > 0 and o2.t == 0.0 and o2.precession
     assert o2.max_torque() < stop * np.sqrt(1 + a * a) / a * 1.0001
     assert o2.energy(T_ALL) < E[0]
+
+
+def _cubic_macrospin(m, Kc1, Ms, c1, c2, alpha=0.0):
+    mat = wl.make_mat(1, Ms=Ms, Kc1=Kc1, alpha=alpha)
+    mat["c1"][:] = c1
+    mat["c2"][:] = c2
+    spec = wl.WorldSpec(name="cubic", grid=(1, 1, 1), cell=(2e-9, 3e-9, 4e-9), S=1, demag=False, mat=mat,
+                        coupling=wl.default_coupling(), m=[np.asarray(m, np.float32).reshape(3, 1, 1, 1)])
+    w = World(spec)
+    w.m = [np.asarray(m, float).reshape(3, 1, 1, 1) / np.linalg.norm(m)]
+    return w
+
+
+def test_P28_cubic_anisotropy_energy_closed_forms():
+    """P:L116 (cubic anisotropy "implemented in the same way as in mumax3"): the first-order cubic energy density is
+    K_c1 (a1^2 a2^2 + a2^2 a3^2 + a3^2 a1^2), a_i the direction cosines on the cubic axes.  Its textbook values --
+    0 along <100>, K_c1/4 along <110>, K_c1/3 along <111> -- are typed in here as numbers; the oracle's energy is
+    -1/4 sum Ms V m.B_cubic, so these fix the product (energy factor 1/4) x (field factor 2 K_c1/Ms), and P10 (field =
+    energy gradient, which fixes their ratio) then fixes each.  The axes are a rotated frame, so a slip in c3 = c1 x c2 or
+    in the index pattern (a_i times the OTHER two squares) shows as well."""
+    from oracle.world import T_ANIS_C
+    Kc1, Ms = 1.0e4, 4.0e5
+    V = 2e-9 * 3e-9 * 4e-9
+    c1 = np.array([2.0, 1.0, 2.0]) / 3.0
+    c2 = np.array([1.0, 2.0, -2.0]) / 3.0
+    c3 = np.cross(c1, c2)
+    for m, want in ((c1, 0.0), (c3, 0.0), (c1 + c2, Kc1 * V / 4), (c2 - c3, Kc1 * V / 4), (c1 + c2 + c3, Kc1 * V / 3),
+                    (c1 - c2 + c3, Kc1 * V / 3)):
+        E = _cubic_macrospin(m, Kc1, Ms, c1, c2).energy(T_ANIS_C)
+        assert abs(E - want) < 1e-12 * Kc1 * V, (m, E, want)
+    # one generic direction: cosines (0.6, 0, 0.8) -> K (0.36 * 0.64) = 0.2304 K
+    E = _cubic_macrospin(0.6 * c1 + 0.8 * c3, Kc1, Ms, c1, c2).energy(T_ANIS_C)
+    assert abs(E - 0.2304 * Kc1 * V) < 1e-12 * Kc1 * V
+
+
+def test_P28_cubic_anisotropy_precession_frequency():
+    """The dynamic pin of the field's prefactor (like P12 for the uniaxial term): for K_c1 > 0 the cubic axes are easy, and a
+    spin tilted by a small angle from c1 precesses about it in the anisotropy field B_A = 2 K_c1 / Ms at omega = gamma B_A
+    (alpha = 0) -- the curvature of K_c1 a1^2 (a2^2 + a3^2) at the axis.  A factor 2 or 1/2 in fields.cubic moves the
+    frequency by that factor; the energy-based pins above cannot see a slip made in both the field and the 1/4."""
+    Kc1, Ms = 6.0e4, 4.0e5
+    c1 = np.array([2.0, 1.0, 2.0]) / 3.0
+    c2 = np.array([1.0, 2.0, -2.0]) / 3.0
+    f_want = GAMMA * (2 * Kc1 / Ms) / (2 * np.pi)          # 8.40 GHz
+    assert abs(f_want - 8.4012e9) < 1e6
+    w = _cubic_macrospin(c1 + 1e-3 * c2, Kc1, Ms, c1, c2)
+    dt, n = 2e-13, 1500                                     # 2.5 periods
+    xs = []
+    for _ in range(n):
+        w.step_dp45_fixed(dt, 1)
+        xs.append(float((w.m[0][:, 0, 0, 0] * c2).sum()))  # component along c2: cos(omega t)
+    xs = np.array(xs)
+    t = dt * np.arange(1, n + 1)
+    zc = np.nonzero(np.sign(xs[1:]) != np.sign(xs[:-1]))[0]
+    tz = t[zc] - xs[zc] * dt / (xs[zc + 1] - xs[zc])
+    assert len(tz) >= 4
+    f_got = 0.5 / np.mean(np.diff(tz))
+    assert abs(f_got - f_want) < 2e-3 * f_want, (f_got, f_want)

@@ -106,7 +106,7 @@ def _toy_world(pbc, seed=3, elastic=False):
         name="toy", grid=grid, cell=(2e-9, 2.5e-9, 1.5e-9), pbc=pbc, S=S,
         regions=rng.integers(0, R, (grid[2], grid[1], grid[0])).astype(np.uint16), mat=mat,
         coupling=wl.default_coupling(A0=-4e-13, A12=-1e-12, D_inter=0.8e-3, scale_A11=0.25, scale_A12=0.5,
-                                     d_homo=(3e4, -2e4, 5e4)),
+                                     d_homo=(3e4, -2e4, 5e4), bc="open"),   # open: the BC of the discrete pair energy (P10)
         bext=(0.05, -0.02, 0.1),
         elastic=dict(C11=2.5e11, C12=1.5e11, C44=1.0e11, rho=6800.0) if elastic else None,
         m=[wl.random_unit(rng, grid), wl.random_unit(rng, grid)],
@@ -495,3 +495,24 @@ def test_P27_neumann_minus_open_is_the_local_boundary_term(hscale):
             want[tuple(sl)] += term[tuple(sl)]
     np.testing.assert_allclose(diff, want, atol=1e-9 * np.abs(want).max())
     assert np.abs(want).max() > 1e-3   # tesla: the term is not negligible at nm cell sizes
+
+
+@pytest.mark.parametrize("S", [1, 2])
+def test_the_default_boundary_is_eq5_and_reduces_to_open_without_dmi(S):
+    """P:L161 "The Neumann boundary conditions as given in Eq. (5) are the default in mumax+": a world that names no
+    boundary kind uses the ghost cells of Eq.5, which matters as soon as there is DMI.  Without any DMI Eq.5 reads
+    2 A11 d_n m = A12 (d_n m' x m) x m, whose solution is d_n m = d_n m' = 0: the default then IS the open boundary."""
+    spec = _neumann_spec((6, 5, 2), S, 23)
+    named, default, opened = spec.copy(), spec.copy(), spec.copy()
+    del default.coupling["bc"]
+    opened.coupling["bc"] = "open"
+    for s in range(S):
+        Bn, Bd, Bo = (World(x).heff(s, terms=T_EXCH | T_DMI | T_A12) for x in (named, default, opened))
+        assert np.array_equal(Bd, Bn)
+        assert np.abs(Bd - Bo).max() > 1e-3 * np.abs(Bo).max()
+    for x in (default, opened):
+        x.mat["D"][:] = 0.0
+        x.coupling["dmi_q"] = None
+    for s in range(S):
+        Bd, Bo = (World(x).heff(s, terms=T_EXCH | T_DMI | T_A12) for x in (default, opened))
+        assert np.abs(Bd - Bo).max() <= 1e-13 * np.abs(Bo).max()
