@@ -150,6 +150,11 @@ const char* mmx_last_error(void);
 
 /* Library version string. */
 const char* mmx_version(void);
+/* Layout revision of this header: raised whenever a struct that crosses the boundary changes size or field order, or an
+ * enumerator changes value (3: mmx_rk_opts carries dt_max, 64 bytes; MMX_F_M2 = 4).  mmx_abi_version() returns the value the
+ * library was built with; a caller compiled against another revision must not pass structs (compare once, at start-up). */
+#define MMX_ABI_VERSION 3
+int mmx_abi_version(void);
 
 /* Create a world on the current CUDA device.
  *   grid[3]     = (Nx, Ny, Nz) cells, each >= 1
@@ -191,12 +196,16 @@ int mmx_set_dmi_tensor(mmx_world* w, int sublattice, const double q[9]);
 
 /* Boundary condition on the non-periodic axes ("The Neumann boundary conditions as given in Eq. (5) are the
  * default in mumax+.  Alternatively, open or periodic boundary conditions can be used").
- *   MMX_BC_OPEN    a stencil pair whose partner is absent (outside the grid, or Ms = 0) adds nothing (reading S9; the
- *                  natural boundary condition of the discrete pair energy; default of this library)
  *   MMX_BC_NEUMANN Eq.5, 2 A11 d_n m = A12 (d_n m' x m) x m + D.(n (x) m), as ghost cells (reading S41): the absent partner of
  *                  every exchange, A12 and DMI pair is m_c + h d_n m, with D.(n (x) m) = m x sum_i n_i q_i and the coupled
- *                  two-sublattice system solved in closed form; it differs from MMX_BC_OPEN by the h-independent local term
- *                  (1/(2 A Ms)) q_i x (m x q_i) on boundary cells (one sublattice).  One or two sublattices. */
+ *                  two-sublattice system solved in closed form.  The default of worlds with one or two sublattices, as in
+ *                  the paper.  Without any DMI constant its solution is d_n m = 0 and the field equals the open one exactly.
+ *   MMX_BC_OPEN    a stencil pair whose partner is absent (outside the grid, or Ms = 0) adds nothing (reading S9; the
+ *                  natural boundary condition of the discrete pair energy).  The default of three-sublattice worlds (Eq.5
+ *                  is written for a sublattice and its partner), opt-in otherwise; BASELINE.json's configurations ask for it
+ *                  in words ("open boundaries").  With DMI it differs from Neumann by the h-independent local field
+ *                  (1/(2 A Ms)) q_i x (m x q_i) on every boundary cell and every cell next to an empty one
+ *                  (one sublattice): about half a tesla for D = 3 mJ/m^2, A = 15 pJ/m, Ms = 580 kA/m. */
 enum { MMX_BC_OPEN = 0, MMX_BC_NEUMANN = 1 };
 int mmx_set_boundary(mmx_world* w, int kind);
 
@@ -331,12 +340,25 @@ int mmx_step_rk4(mmx_world* w, double dt, long long nsteps);
  *     the next attempt and abandon that attempt (it counts neither as accepted nor as rejected).
  *   - the error estimate is taken over the magnetic variables only (the paper leaves adaptive
  *     stepping of the elastic variables to future work).  With elastodynamics on, adaptive
- *     stepping therefore clamps the step to dt_max, and dt_max <= 0 then selects
- *     0.5 min(cellsize) / sqrt(C11 / rho) (half the explicit stability bound of the fastest
- *     elastic wave), so that a quiet magnet cannot drive dt past the elastic limit.
+ *     stepping therefore clamps the step to dt_max, and dt_max <= 0 then selects the bound of the chosen method,
+ *         dt_max = 0.9 y_max / omega_max,
+ *     y_max = mmx_rk_imag_stability_limit(method, 1e-6), omega_max = 1.3722 v_max sqrt(sum_a 1/h_a^2) over the axes with
+ *     more than one cell: 1.3722/h is the largest wave number the fourth-order first difference of Eq.7 can
+ *     represent, v_max the fastest wave of the cubic medium (the largest of sqrt(C11/rho), sqrt(C44/rho) and the
+ *     longitudinal velocities along [110] and [111]).  An undamped wave sits on the imaginary axis of the method's
+ *     stability region; above y_max every step amplifies round-off, so a quiet magnet must not drive dt past it.
+ *     Heun, Cash-Karp and Fehlberg are nowhere neutrally stable on that axis: their bound comes from the growth allowance
+ *     (1e-6 per step) alone and is 2 to 20 times smaller than Dormand-Prince's.
  *   - MMX_ENAN: a NaN/Inf reached the error or torque reduction; the attempt is not accepted, the
  *     accepted state and time are left as they were, stepping stops. */
 int mmx_step_rk45(mmx_world* w, const mmx_rk_opts* opts, mmx_rk_stats* stats);
+
+/* Host-only helper, needs no GPU: how far up the imaginary axis a step of `method` (Table 2, or MMX_RK4) may
+ * reach.  *y_max = the largest y with |R(i y')| <= 1 + growth for all 0 <= y' <= y, R the method's stability polynomial;
+ * an undamped oscillation of angular frequency omega advanced with omega dt <= y_max is amplified by at most 1 + growth per
+ * step.  growth = 0: RK4 2 sqrt 2, Bogacki-Shampine sqrt 3, Dormand-Prince 0.997, (almost) 0 for Heun, Cash-Karp, Fehlberg.
+ * Resolution 1e-4, searched up to y = 4. */
+int mmx_rk_imag_stability_limit(int method, double growth, double* y_max);
 
 /* Relaxation ("after letting a non-collinear antiferromagnet relax from a random state"; DESIGN.md reading
  * S39): the precession term m x B of Eq.2 is dropped and the damping term -gamma alpha/(1+alpha^2) m x (m x B) is

@@ -15,6 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmmx.so")
 
 HOST, DEVICE = 0, 1
+ABI_VERSION = 3   # MMX_ABI_VERSION of include/mmx.h
 T_EXCH, T_DMI, T_ANIS_U, T_ANIS_C, T_ZEEMAN, T_DEMAG, T_A12, T_A0, T_DMI_INTER, T_MEL, T_DMI_HOMO = (
     1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1024)
 T_ALL = 2047
@@ -76,6 +77,7 @@ _W = C.c_void_p
 PROTOTYPES = {
     "mmx_last_error": (C.c_char_p, []),
     "mmx_version": (C.c_char_p, []),
+    "mmx_abi_version": (C.c_int, []),
     "mmx_world_create": (C.c_int, [_I3, _D3, _I3, C.c_int, C.c_void_p, C.POINTER(_W)]),
     "mmx_world_destroy": (C.c_int, [_W]),
     "mmx_set_regions": (C.c_int, [_W, C.c_void_p, C.c_int, C.c_int]),
@@ -104,6 +106,7 @@ PROTOTYPES = {
     "mmx_max_torque": (C.c_int, [_W, _D3]),
     "mmx_step_rk4": (C.c_int, [_W, C.c_double, C.c_longlong]),
     "mmx_step_rk45": (C.c_int, [_W, C.POINTER(RkOpts), C.POINTER(RkStats)]),
+    "mmx_rk_imag_stability_limit": (C.c_int, [C.c_int, C.c_double, _D3]),
     "mmx_stray_field": (C.c_int, [_W, C.c_double, C.c_void_p, C.c_int]),
     "mmx_stray_field_static": (C.c_int, [_I3, C.c_int, _D3, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "mmx_stray_table_host": (C.c_int, [_I3, _D3, C.c_double, C.c_void_p, C.c_longlong]),
@@ -134,6 +137,9 @@ def load(path: str | None = None):
         fn = getattr(lib, name)
         fn.restype = res
         fn.argtypes = args
+    if lib.mmx_abi_version() != ABI_VERSION:
+        raise RuntimeError("%s was built from another revision of include/mmx.h (library %d, binding %d): rebuild it"
+                           % (p, lib.mmx_abi_version(), ABI_VERSION))
     if path is None:
         _lib = lib
     return lib
@@ -178,6 +184,14 @@ def kernel_spectrum_host(grid, cell, pbc=(0, 0, 0), cutoff_cells=32.0):
     out = np.empty((6, kz, ky, xp), dtype=np.float32)
     _check(lib.mmx_kernel_spectrum_host(*a, float(cutoff_cells), out.ctypes.data, out.size, dims))
     return out, (px, py, pz)
+
+
+def rk_imag_stability_limit(method, growth=0.0) -> float:
+    """mmx_rk_imag_stability_limit: largest omega*dt of an undamped oscillation the method advances with an amplification
+    of at most 1 + growth per step; needs no GPU."""
+    y = C.c_double()
+    _check(load().mmx_rk_imag_stability_limit(int(method), float(growth), C.byref(y)))
+    return y.value
 
 
 STRAY_STATIC_MAX_CELLS = 262144

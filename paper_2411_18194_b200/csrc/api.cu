@@ -50,6 +50,61 @@ void default_material(mmx_material* m) {
   m->c2[1] = 1.0;
 }
 
+// Largest y such that |R(i y')| <= 1 + growth for all y' in [0, y], R the stability polynomial of the tableau,
+// R(z) = 1 + sum_k z^k b^T A^(k-1) 1: how far up the imaginary axis (undamped waves, u'' = -omega^2 u, y = omega dt) a step
+// may reach before round-off is amplified by more than `growth` per step.  RK4: 2 sqrt 2; Bogacki-Shampine: sqrt 3;
+// Dormand-Prince: 0.997; Heun, Cash-Karp and Fehlberg are not neutrally stable anywhere on the axis (|R| - 1 ~ y^4 / y^6),
+// so their limit is set by the growth allowance alone.  Scanned in steps of 1e-4 up to y = 4.
+double imag_axis_limit(const MmxTableau& t, double growth) {
+  const int s = t.stages;
+  double coef[MMX_MAX_STAGES + 1], v[MMX_MAX_STAGES], nv[MMX_MAX_STAGES];
+  coef[0] = 1.0;
+  for (int i = 0; i < s; ++i) v[i] = 1.0;
+  for (int k = 1; k <= s; ++k) {
+    double d = 0.0;
+    for (int i = 0; i < s; ++i) d += t.b[i] * v[i];
+    coef[k] = d;
+    for (int i = 0; i < s; ++i) {
+      nv[i] = 0.0;
+      for (int j = 0; j < i; ++j) nv[i] += t.a[i][j] * v[j];
+    }
+    for (int i = 0; i < s; ++i) v[i] = nv[i];
+  }
+  double last = 0.0;
+  for (int q = 1; q <= 40000; ++q) {
+    const double y = 1e-4 * q;
+    double re = 0.0, im = 0.0, p = 1.0;  // p = y^k
+    for (int k = 0; k <= s; ++k) {
+      switch (k & 3) { case 0: re += coef[k] * p; break; case 1: im += coef[k] * p; break;
+                       case 2: re -= coef[k] * p; break; default: im -= coef[k] * p; }
+      p *= y;
+    }
+    if (sqrt(re * re + im * im) > 1.0 + growth + 1e-13) break;
+    last = y;
+  }
+  return last;
+}
+
+// Step bound of adaptive stepping with elastodynamics on: dt_max = 0.9 y_max / omega_max.
+//   y_max      imag_axis_limit of the method with a growth allowance of 1e-6 per step
+//   omega_max  largest frequency of the discrete elastic operator: the fourth-order central first derivative applied twice
+//              (Eq.7) has the symbol (8 sin th - sin 2th)/(6 h) <= 1.3722 / h per axis, so
+//              omega_max <= 1.3722 v_max sqrt(sum over axes with more than one cell of 1 / h_a^2); v_max the fastest wave
+//              of the cubic medium, the largest of the longitudinal velocities along [100], [110], [111] and sqrt(C44/rho)
+double elastic_dt_limit(const mmx_world* w, const MmxTableau& tab) {
+  const double C11 = w->el.C11, C12 = w->el.C12, C44 = w->el.C44;
+  double c = C11;
+  if (C44 > c) c = C44;
+  if (0.5 * (C11 + C12 + 2 * C44) > c) c = 0.5 * (C11 + C12 + 2 * C44);
+  if ((C11 + 2 * C12 + 4 * C44) / 3.0 > c) c = (C11 + 2 * C12 + 4 * C44) / 3.0;
+  double k2 = 0.0;
+  for (int a = 0; a < 3; ++a)
+    if (w->grid[a] > 1) k2 += 1.0 / (w->cell[a] * w->cell[a]);
+  if (!(c > 0) || !(w->el.rho > 0) || !(k2 > 0)) return 0.0;
+  const double omega_max = 1.3722 * sqrt(c / w->el.rho) * sqrt(k2);
+  return 0.9 * imag_axis_limit(tab, 1e-6) / omega_max;
+}
+
 size_t vecN(const mmx_world* w) { return (size_t)w->nvec * 3 * w->N; }
 
 // ---- tableaux (Table 2; classical RK4 from the textbook reference [51]) -----------
@@ -269,7 +324,12 @@ void fill_local(const mmx_world* w, LocalArgs& a, unsigned terms) {
   a.terms = terms;
   a.has_J = (w->J[0] != 0.0 || w->J[1] != 0.0 || w->J[2] != 0.0) ? 1 : 0;
   a.relax = w->relax_mode ? 1 : 0;
-  a.neumann = w->boundary == MMX_BC_NEUMANN ? 1 : 0;
+  // Eq.5 without any DMI has the solution d_n m = d_n m' = 0: every ghost equals its cell, exchange and A12 pairs with a
+  // ghost add exactly zero, and the field is that of the open boundary bit for bit.  Ghost cells are therefore formed only
+  // when some DMI constant is set (the default boundary then costs nothing on the worlds without DMI).
+  bool any_dmi = w->has_dmiq || w->cpl.D_inter != 0.0;
+  for (size_t q = 0; q < w->mats.size() && !any_dmi; ++q) any_dmi = w->mats[q].D != 0.0;
+  a.neumann = (w->boundary == MMX_BC_NEUMANN && any_dmi) ? 1 : 0;
   a.bdemag = (terms & MMX_T_DEMAG) ? w->bdemag : nullptr;
   a.strain = (terms & MMX_T_MEL) ? w->strain : nullptr;
   a.ctrl = w->d_ctrl;
@@ -389,11 +449,8 @@ int run_steps(mmx_world* w, const mmx_rk_opts* o, mmx_rk_stats* stats) {
   h.dt = o->dt0 > 0 ? o->dt0 : 0.0;
   h.dt_max = o->dt_max > 0 ? o->dt_max : 0.0;
   if (w->has_elastic && !o->fixed_dt && !(h.dt_max > 0)) {
-    // the error estimate covers the magnetic variables only: keep dt inside the elastic limit
-    double hmin = 1e300;
-    for (int a = 0; a < 3; ++a)
-      if (w->grid[a] > 1 && w->cell[a] < hmin) hmin = w->cell[a];
-    if (hmin < 1e300 && w->el.C11 > 0) h.dt_max = 0.5 * hmin / sqrt(w->el.C11 / w->el.rho);
+    // the error estimate covers the magnetic variables only: keep dt inside the elastic limit of this method
+    h.dt_max = elastic_dt_limit(w, tab);
   }
   h.tol = o->tol > 0 ? o->tol : 1e-5;
   h.t_end = o->t_end > 0 ? o->t_end : 0.0;
@@ -583,7 +640,16 @@ int mmx_fail(int code, const char* fmt, ...) {
 extern "C" {
 
 const char* mmx_last_error(void) { return g_err; }
-const char* mmx_version(void) { return "mmx 0.1 (sm_100a)"; }
+const char* mmx_version(void) { return "mmx 0.3 (sm_100a)"; }
+int mmx_abi_version(void) { return MMX_ABI_VERSION; }
+
+int mmx_rk_imag_stability_limit(int method, double growth, double* y_max) {
+  if (!y_max) return mmx_fail(MMX_EINVAL, "NULL argument");
+  if (method < MMX_RK4 || method > MMX_RKF45) return mmx_fail(MMX_EINVAL, "unknown method %d", method);
+  if (!(growth >= 0)) return mmx_fail(MMX_EINVAL, "growth must be >= 0");
+  *y_max = imag_axis_limit(make_tableau(method), growth);
+  return MMX_OK;
+}
 
 int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[3], int n_sublattices,
                      void* cuda_stream, mmx_world** out) {
@@ -621,6 +687,9 @@ int mmx_world_create(const int grid[3], const double cellsize[3], const int pbc[
     for (int k = 0; k < 9; ++k) w->dmiq[s][k] = 0.0;
   memset(&w->sl, 0, sizeof(w->sl));
   w->relax_mode = false;
+  // P:L161 "The Neumann boundary conditions as given in Eq. (5) are the default in mumax+"; Eq.5 is written for a
+  // sublattice and its partner, so a three-sublattice world starts open (mmx_set_boundary refuses Neumann there)
+  w->boundary = n_sublattices <= 2 ? MMX_BC_NEUMANN : MMX_BC_OPEN;
   w->n_tmaps = 0;
   w->step_graph = nullptr; w->graph_method = -1; w->graph_epoch = -1; w->cfg_epoch = 0; w->graph_launches = 0;
   w->use_graphs = getenv("MMX_NO_GRAPH") == nullptr;
@@ -791,7 +860,6 @@ int mmx_set_slonczewski(mmx_world* w, const mmx_slonczewski* sl) {
   if (!w) return mmx_fail(MMX_EINVAL, "NULL world");
   if (!sl) {
     memset(&w->sl, 0, sizeof(w->sl));
-  w->relax_mode = false;
   } else {
     const double n = sqrt(sl->mp[0] * sl->mp[0] + sl->mp[1] * sl->mp[1] + sl->mp[2] * sl->mp[2]);
     if (sl->jz != 0.0 && !(n > 0)) return mmx_fail(MMX_EINVAL, "Slonczewski torque needs a fixed-layer direction mp");

@@ -1016,10 +1016,11 @@ __global__ void __launch_bounds__(256) k_dot_energy(const float* m, const float*
 
 }  // namespace
 
-// tensor map of a state buffer [3 nvec][nz][ny][nx] floats with the halo box of k_local_t
-static int tmap_for(mmx_world* w, const float* base, const CUtensorMap** out) {
+// tensor map of a state buffer [3 nvec][nz][ny][nx] floats with the halo box of k_local_t, returned by value: a later
+// lookup that misses on a full cache recycles slot 0, so a pointer into the cache would not survive a second call
+static int tmap_for(mmx_world* w, const float* base, CUtensorMap* out) {
   for (int k = 0; k < w->n_tmaps; ++k)
-    if (w->tmaps[k].base == base) { *out = reinterpret_cast<const CUtensorMap*>(w->tmaps[k].bytes); return MMX_OK; }
+    if (w->tmaps[k].base == base) { *out = *reinterpret_cast<const CUtensorMap*>(w->tmaps[k].bytes); return MMX_OK; }
   if (w->n_tmaps >= 4) w->n_tmaps = 0;
   static PFN_cuTensorMapEncodeTiled encode = nullptr;
   if (!encode) {
@@ -1040,7 +1041,7 @@ static int tmap_for(mmx_world* w, const float* base, const CUtensorMap** out) {
   if (r != CUDA_SUCCESS) return mmx_fail(MMX_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
   t.base = base;
   w->n_tmaps++;
-  *out = reinterpret_cast<const CUtensorMap*>(t.bytes);
+  *out = *reinterpret_cast<const CUtensorMap*>(t.bytes);
   return MMX_OK;
 }
 
@@ -1056,10 +1057,9 @@ int mmx_local_launch(mmx_world* w, const LocalArgs& a) {
   const bool open_all = !a.per[0] && !a.per[1] && !a.per[2];
   if (uniform && w->S == 1 && open_all) {
     // TMA halo tiles (k_local_t)
-    const CUtensorMap *m0, *m1;
-    if (int rc = tmap_for(w, a.yin[0], &m0)) return rc;
-    if (int rc = tmap_for(w, a.yin[1], &m1)) return rc;
-    const CUtensorMap t0 = *m0, t1 = *m1;  // (copies: a second lookup may recycle the cache slot)
+    CUtensorMap t0, t1;
+    if (int rc = tmap_for(w, a.yin[0], &t0)) return rc;
+    if (int rc = tmap_for(w, a.yin[1], &t1)) return rc;
     const dim3 grid((w->grid[0] + LT_TX - 1) / LT_TX, (w->grid[1] + LT_TY - 1) / LT_TY, (w->grid[2] + LT_TZ - 1) / LT_TZ);
     const int mode = (a.ynext[0] ? 1 : 0) | (a.do_err ? 2 : 0);
 #define MMX_LT_GO(NP_, M_)                                                                                         \

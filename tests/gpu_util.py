@@ -55,4 +55,4 @@ def pair_oracle(spec, demag_mode="fft"):
 
 
 def gpu_m(g, S):
-    return [g.get_state(mmx.F_M0 + s) for s in range(S)]
+    return [g.get_state(mmx.F_M[s]) for s in range(S)]

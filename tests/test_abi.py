@@ -99,3 +99,32 @@ def test_padding_rule():
     assert P == (64, 32, 8)
     _, P = mmx.kernel_spectrum_host((1, 1, 1), (1e-9,) * 3)
     assert P == (2, 1, 1)
+
+
+def test_imaginary_axis_stability_limits_of_the_tableaux(lib):
+    """mmx_rk_imag_stability_limit (the elastic step bound of mmx_step_rk45): closed forms where they exist -- RK4
+    |R(iy)|^2 = 1 - y^6/72 + y^8/576 <= 1 up to 2 sqrt 2, Bogacki-Shampine 1 - y^4/12 + y^6/36 <= 1 up to sqrt 3, Heun
+    |R|^2 = 1 + y^4/4 -- and for every method the stability polynomial of the oracle's exact-fraction tableau (Table 2,
+    P:L122-131) evaluated independently on both sides of the returned limit."""
+    from oracle import rk
+    assert abs(mmx.rk_imag_stability_limit(mmx.RK4) - 2 * np.sqrt(2)) < 1.5e-4
+    assert abs(mmx.rk_imag_stability_limit(mmx.BS23) - np.sqrt(3)) < 1.5e-4
+    g = 1e-6
+    assert abs(mmx.rk_imag_stability_limit(mmx.HEUN12, g) - (4 * ((1 + g) ** 2 - 1)) ** 0.25) < 1.5e-4
+    tabs = {mmx.RK4: rk.RK4, mmx.DP45: rk.DP45, mmx.HEUN12: rk.HEUN12, mmx.BS23: rk.BS23, mmx.CK45: rk.CK45, mmx.RKF45: rk.RKF45}
+    for method, tab in tabs.items():
+        s = tab.stages
+        A = np.zeros((s, s))
+        for i, row in enumerate(tab.a):
+            A[i, :len(row)] = [float(x) for x in row]
+        b = np.array([float(x) for x in tab.b])
+        R = lambda y: abs(1 + 1j * y * (b @ np.linalg.solve(np.eye(s) - 1j * y * A, np.ones(s))))
+        for growth in (0.0, 1e-6):
+            y = mmx.rk_imag_stability_limit(method, growth)
+            assert 0 <= y < 3.0
+            if y > 0:
+                assert max(R(t) for t in np.linspace(0, y, 400)) <= 1 + growth + 1e-12, (method, growth)
+            assert R(y + 2e-4) > 1 + growth, (method, growth)
+    assert mmx.rk_imag_stability_limit(mmx.DP45) < 1.0 < mmx.rk_imag_stability_limit(mmx.BS23)
+    with pytest.raises(mmx.MmxError):
+        mmx.rk_imag_stability_limit(17)

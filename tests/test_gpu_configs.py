@@ -121,7 +121,7 @@ def test_full_protocol_against_stored_oracle_trajectory(case):
         np.testing.assert_allclose((m.astype(np.float64) ** 2).sum(axis=0), 1.0, atol=2e-6)
     else:
         for s in range(spec.S):
-            m = g.get_state(mmx.F_M0 + s)
+            m = g.get_state(mmx.F_M[s])
             d = max_dm(m, gold["m%d" % s])
             assert d <= TRAJ_TOL, (case, s, d)
             np.testing.assert_allclose((m.astype(np.float64) ** 2).sum(axis=0), 1.0, atol=2e-6)

@@ -30,6 +30,8 @@ def _rich_spec(name, grid, seed=7):
         spec.mat["B2"][s] = -0.7e7
         spec.mat["A"][s] = 1e-11 * (1 + 0.3 * rng.random(R))
     spec.bext = (0.01, -0.02, 0.1)
+    spec.coupling.setdefault("bc", "open")    # (c5 names no boundary kind; with the DMI added here the default would be Eq.5,
+    #                                            which has tests of its own in test_gpu_next.py)
     if spec.S == 2:
         spec.coupling.update(A0=-4e-13, A12=-1e-12, D_inter=0.5e-3, scale_A11=0.25, scale_A12=0.5,
                              d_homo=(3e4, -2e4, 5e4))
@@ -321,7 +323,7 @@ def test_viscous_elastic_damping_acceleration_and_trajectory():
     g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=100)
     o.step_dp45_fixed(dt, 100)
     for s_ in range(spec.S):
-        assert np.abs(g.get_state(mmx.F_M0 + s_).astype(np.float64) - o.m[s_]).max() <= 1e-4
+        assert np.abs(g.get_state(mmx.F_M[s_]).astype(np.float64) - o.m[s_]).max() <= 1e-4
     u, v = g.get_state(mmx.F_U), g.get_state(mmx.F_V)
     assert np.abs(u - o.u).max() <= 1e-4 * max(np.abs(o.u).max(), 1e-30)
     assert np.abs(v - o.v).max() <= 1e-4 * max(np.abs(o.v).max(), 1e-30)
@@ -352,7 +354,7 @@ def test_general_dmi_tensor(name, grid, pbc):
     g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=20)
     o.step_dp45_fixed(dt, 20)
     for s in range(spec.S):
-        assert np.abs(g.get_state(mmx.F_M0 + s).astype(np.float64) - o.m[s]).max() <= 1e-4
+        assert np.abs(g.get_state(mmx.F_M[s]).astype(np.float64) - o.m[s]).max() <= 1e-4
     g.destroy()
 
 

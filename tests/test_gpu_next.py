@@ -35,7 +35,7 @@ def test_slonczewski_torque_and_trajectory(name, grid):
     g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=30)
     o.step_dp45_fixed(dt, 30)
     for s in range(spec.S):
-        assert max_dm(g.get_state(mmx.F_M0 + s), o.m[s]) <= TRAJ_TOL
+        assert max_dm(g.get_state(mmx.F_M[s]), o.m[s]) <= TRAJ_TOL
     # clearing it restores the plain torque
     g.set_slonczewski(jz=0.0)
     g.set_state(mmx.F_M0, np.ascontiguousarray(spec.m[0], dtype=np.float32))
@@ -100,7 +100,7 @@ def test_inter_sublattice_dmi_tensor(grid, pbc):
     g.step_rk45(method=mmx.DP45, fixed_dt=True, dt0=dt, nsteps=20)
     o.step_dp45_fixed(dt, 20)
     for s in range(2):
-        assert max_dm(g.get_state(mmx.F_M0 + s), o.m[s]) <= TRAJ_TOL
+        assert max_dm(g.get_state(mmx.F_M[s]), o.m[s]) <= TRAJ_TOL
     g.destroy()
 
 
@@ -310,3 +310,31 @@ def test_neumann_boundary_condition(name, grid, pbc):
     mag = (o.p[0]["Ms"] > 0)[None]
     assert field_err(g.eval_heff(0, mmx.T_EXCH | mmx.T_DMI), o_open.heff(0, terms=oc.T_EXCH | oc.T_DMI) * mag) < FIELD_TOL
     g.destroy()
+
+
+@pytest.mark.parametrize("name,grid", [("c1", (24, 12, 1)), ("c3", (32, 16, 1))])
+def test_default_boundary_is_neumann(name, grid):
+    """Eq.5 is the default.  A world on which mmx_set_boundary is never called (one or two sublattices, DMI
+    present) gives the oracle's default, which is the Neumann field and not the open one; with every DMI constant zero
+    the default is the open boundary bit for bit (and stays on the kernels of the open case)."""
+    spec = _rich_spec(name, grid, seed=61)
+    spec.coupling.pop("bc", None)
+    g, o = pair(spec)
+    so = spec.copy()
+    so.coupling["bc"] = "open"
+    from gpu_util import pair_oracle
+    o_open = pair_oracle(so)
+    for s in range(spec.S):
+        mag = (o.p[s]["Ms"] > 0)[None]
+        assert field_err(o_open.heff(s) * mag, o.heff(s) * mag) > 1e-3
+        assert field_err(g.eval_heff(s, mmx.T_ALL), o.heff(s) * mag) < FIELD_TOL, (name, s)
+    g.destroy()
+    for sp in (spec, so):
+        sp.mat["D"][:] = 0.0
+        sp.coupling["D_inter"] = 0.0
+        sp.coupling["dmi_q"] = None
+        sp.coupling.pop("dmi_q12", None)
+    gd, go = mmx.World.from_spec(spec), mmx.World.from_spec(so)
+    for s in range(spec.S):
+        assert np.array_equal(gd.eval_heff(s, mmx.T_ALL), go.eval_heff(s, mmx.T_ALL))
+    gd.destroy(); go.destroy()

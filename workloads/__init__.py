@@ -80,6 +80,8 @@ def make_mat(S: int, R: int = 1, **kw) -> dict:
 def default_coupling(**kw) -> dict:
     c = dict(A0=0.0, A12=0.0, latcon=0.35e-9, D_inter=0.0, scale_A11=1.0, scale_A12=1.0,
              d_homo=(0.0, 0.0, 0.0), dmi_q=None)   # dmi_q: [S][3][3] per-axis DMI vectors of Eq.4, J/m^2
+    # bc: "open" | "neumann"; absent = the paper's default (Eq.5 for one or two sublattices).  BASELINE.json's
+    # configurations 1, 3 and 4 say "open boundaries" in words, so their specs carry bc="open".
     c.update(kw)
     return c
 
@@ -177,7 +179,7 @@ def c1(grid=(64, 16, 1), seed=1001) -> WorldSpec:
     rng = np.random.default_rng(seed)
     return WorldSpec(
         name="c1", grid=tuple(grid), cell=(7.8125e-9, 7.8125e-9, 3e-9),
-        mat=make_mat(1, Ms=8.0e5, A=1.3e-11, alpha=0.5), coupling=default_coupling(),
+        mat=make_mat(1, Ms=8.0e5, A=1.3e-11, alpha=0.5), coupling=default_coupling(bc="open"),   # "open boundaries"
         m=[random_unit(rng, grid)],
         integrator=dict(method="rk4", dt=1e-13, nsteps=2000))
 
@@ -188,7 +190,9 @@ def c2(grid=(256, 256, 1), seed=1002) -> WorldSpec:
     return WorldSpec(
         name="c2", grid=tuple(grid), cell=(2e-9, 2e-9, 1e-9), pbc=(4, 4, 0),
         mat=make_mat(1, Ms=5.8e5, A=1.5e-11, D=3.0e-3, Ku1=8.0e5, alpha=0.3),
-        coupling=default_coupling(), bext=(0.0, 0.0, 0.1),
+        # "periodic in-plane"; the one-cell z axis has no stencil partner and interfacial DMI no z term, so the
+        # boundary kind is immaterial there: stated as open, which keeps the periodic fast kernels in the tests
+        coupling=default_coupling(bc="open"), bext=(0.0, 0.0, 0.1),
         m=[smoothed_random_unit(rng, grid, 3.0)],
         integrator=dict(method="dp45", dt=2e-14, nsteps=500, tol=1e-5))
 
@@ -210,7 +214,7 @@ def c3(grid=(1024, 128, 1), seed=1003, grain_diameter=20e-9) -> WorldSpec:
     m1 = neel_wall(grid, cell, x0, width)
     return WorldSpec(
         name="c3", grid=tuple(grid), cell=cell, S=2, regions=regions, mat=mat,
-        coupling=default_coupling(A0=-4.0e-13, A12=-1.0e-12, latcon=0.35e-9, D_inter=0.0),
+        coupling=default_coupling(A0=-4.0e-13, A12=-1.0e-12, latcon=0.35e-9, D_inter=0.0, bc="open"),   # "open boundaries"
         J=(1e12, 0.0, 0.0), m=[m1, (-m1).astype(np.float32)],
         integrator=dict(method="dp45", dt=5e-15, nsteps=400))
 
@@ -220,7 +224,7 @@ def c4(grid=(256, 256, 64), seed=1004) -> WorldSpec:
     rng = np.random.default_rng(seed)
     return WorldSpec(
         name="c4", grid=tuple(grid), cell=(4e-9, 4e-9, 4e-9),
-        mat=make_mat(1, Ms=1.0e6, A=1.0e-11, alpha=0.1), coupling=default_coupling(),
+        mat=make_mat(1, Ms=1.0e6, A=1.0e-11, alpha=0.1), coupling=default_coupling(bc="open"),   # "open boundaries"
         m=[random_unit(rng, grid)],
         integrator=dict(method="dp45", dt=1e-13, nsteps=100))
 
