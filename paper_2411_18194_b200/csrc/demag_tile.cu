@@ -26,6 +26,7 @@
 // stays linear -- which makes the column-pair reads of eight different rows conflict-free; the kernel
 // images are swizzled with ((kz >> 1) & 7) for the same reason.
 #include "fft_reg.cuh"
+#include "mbar.cuh"
 #include "mmx_internal.h"
 
 using namespace mmxreg;
@@ -68,7 +69,8 @@ __device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
 __device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s32(bar)), "r"(bytes) : "memory");
 }
-// wait for the phase with the given parity; a tile that never lands traps instead of hanging the GPU
+// wait for the phase with the given parity; after 65 536 failed polls the wait backs off and is bounded by wall time
+// (mbar.cuh): a slow tile is waited for, a tile that has not landed after 10 s traps instead of hanging the GPU
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
   unsigned ok = 0;
   for (int spin = 0; !ok; ++spin) {
@@ -77,7 +79,7 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
         "selp.u32 %0, 1, 0, p;\n}\n"
         : "=r"(ok) : "r"(s32(bar)), "r"(parity) : "memory");
-    if (!ok && spin > (1 << 22)) __trap();
+    if (!ok && spin > (1 << 16)) { mmx_mbar_wait_slow(s32(bar), parity); return; }
   }
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {

@@ -23,6 +23,7 @@
 
 #include <cstdio>
 
+#include "mbar.cuh"
 #include "mmx_internal.h"
 
 namespace {
@@ -722,7 +723,7 @@ __global__ void __launch_bounds__(LT_NT, 3) k_local_t(LocalArgs a, const __grid_
     for (int spin = 0; !ok; ++spin) {
       asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}\n"
                    : "=r"(ok) : "r"(lt_s32(&bar)) : "memory");
-      if (!ok && spin > (1 << 22)) __trap();
+      if (!ok && spin > (1 << 16)) { mmx_mbar_wait_slow(lt_s32(&bar), 0); break; }   // (mbar.cuh: back-off, 10 s wall-time bound)
     }
   }
   float errv = 0.f, tqv = 0.f;
