@@ -35,6 +35,21 @@ def torque_err_conditioned(got, ref, B, alpha, gamma):
     return float((d / scale).max())
 
 
+EST_RTOL = 1e-3   # embedded error estimate of a fixed-step run, relative (SURVEY 8d "rel. 1e-3")
+
+
+def assert_estimates(got, ref, floor):
+    """Error-estimate history of a fixed-step run against the oracle's: |got - ref| <= EST_RTOL ref + floor, floor the
+    absolute fp32 rounding floor of the estimate derived in DESIGN.md section 10 (passed in by the test).  Wherever the
+    estimate is >= 100 floor this is a relative comparison at 1e-3 (+ at most 1e-2 from the floor); floor-limited entries
+    are held by the floor alone.  On failure the message carries the measured ratio."""
+    got, ref = np.asarray(got, np.float64), np.asarray(ref, np.float64)
+    assert got.shape == ref.shape
+    d = np.abs(got - ref)
+    worst = float(((d - floor) / np.maximum(ref, 1e-300)).max())
+    assert (d <= EST_RTOL * ref + floor).all(), "estimate history: max (|d| - floor) / est = %.3g, bar %.1g" % (worst, EST_RTOL)
+
+
 def max_dm(a, b):
     return float(np.abs(np.asarray(a, np.float64) - np.asarray(b, np.float64)).max())
 

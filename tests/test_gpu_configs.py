@@ -15,7 +15,7 @@ import paper_2411_18194_b200 as mmx
 import workloads as wl
 from oracle import constants as oc
 from oracle import rk as ork
-from gpu_util import FIELD_TOL, TRAJ_TOL, field_err, max_dm, pair, torque_err_conditioned
+from gpu_util import assert_estimates, FIELD_TOL, TRAJ_TOL, field_err, max_dm, pair, torque_err_conditioned
 from test_gpu_fields import TERMS, _rich_spec
 
 pytestmark = pytest.mark.gpu
@@ -111,7 +111,7 @@ def test_full_protocol_against_stored_oracle_trajectory(case):
         assert st["accepted"] == n and st["rejected"] == 0
         hist = g.get_err_history(n)
         assert len(hist) == n
-        np.testing.assert_allclose(hist, gold["errs"], rtol=2e-2, atol=max(floor, 1e-9))
+        assert_estimates(hist, gold["errs"], max(floor, 1e-9))
     assert abs(g.get_time() - n * dt) < 1e-6 * n * dt
     if name == "c4":
         idx = gold["mask_index"]

@@ -6,7 +6,7 @@ import pytest
 
 import paper_2411_18194_b200 as mmx
 import workloads as wl
-from gpu_util import TRAJ_TOL, gpu_m, max_dm, pair, pair_oracle
+from gpu_util import assert_estimates, TRAJ_TOL, gpu_m, max_dm, pair, pair_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -50,7 +50,7 @@ def test_dp45_fixed_step_trajectory(name, grid, nsteps):
     # the combination weights it with sum_j |e_j| = 0.16 (Dormand-Prince, Table 2):
     #   atol = 16 * 2^-24 * 0.16 * dt * gamma * max|B_eff|
     atol = 16 * 2.0 ** -24 * 0.16 * dt * 1.7595e11 * bmax
-    np.testing.assert_allclose(hist, errs, rtol=2e-2, atol=max(atol, 1e-9))
+    assert_estimates(hist, errs, max(atol, 1e-9))
     if spec.elastic is not None:
         u, v = g.get_state(mmx.F_U), g.get_state(mmx.F_V)
         assert np.abs(u - o.u).max() <= 1e-4 * max(np.abs(o.u).max(), 1e-30)
