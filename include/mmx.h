@@ -181,7 +181,7 @@ int mmx_set_regions(mmx_world* w, const uint16_t* region_of_cell, int mem, int n
 /* Material of (sublattice, region); call after mmx_set_regions. */
 int mmx_set_material(mmx_world* w, int sublattice, int region, const mmx_material* mat);
 int mmx_set_coupling(mmx_world* w, const mmx_coupling* c);
-int mmx_set_bext(mmx_world* w, const double B[3]);     /* uniform external field, T */
+int mmx_set_bext(mmx_world* w, const double B[3]);     /* uniform external (Zeeman) field, T */
 int mmx_set_current(mmx_world* w, const double J[3]);  /* Zhang-Li current density, A/m^2 */
 /* General intra-sublattice DMI of Eq.4: eps = sum_ijk D_ijk m_j d_i m_k, D_ijk = -D_ikj
  * (9 independent components).  q[3*i + l] is component l of the vector q_i of axis i, J/m^2, with
@@ -227,7 +227,8 @@ int mmx_set_elastic(mmx_world* w, const mmx_elastic* e);
 /* Switch the magnetostatic term on/off for stepping (default on once the kernel exists). */
 int mmx_enable_demag(mmx_world* w, int on);
 
-/* Copy a state field in / out: `field` = MMX_F_*; buf is fp32 [3][Nz][Ny][Nx]. */
+/* Copy a state field in / out: `field` = MMX_F_*; buf is fp32 [3][Nz][Ny][Nx] (the user's side of the state is
+ * plain arrays).  m is taken as given: the caller passes unit vectors (or 0 in cells without a magnet). */
 int mmx_set_state(mmx_world* w, int field, const float* buf, int mem);
 int mmx_get_state(mmx_world* w, int field, float* buf, int mem);
 int mmx_set_time(mmx_world* w, double t);
@@ -267,11 +268,13 @@ int mmx_eval_heff(mmx_world* w, int sublattice, unsigned term_mask, float* out, 
 int mmx_eval_torque(mmx_world* w, int sublattice, float* out, int mem);
 /* Elastic right-hand side: acceleration (f_el + sum_s f_mel)/rho  (Eq.7-8), m/s^2. */
 int mmx_eval_accel(mmx_world* w, float* out, int mem);
-/* Energy (J) of the terms in term_mask summed over sublattices, fp64 accumulation. */
+/* Energy (J) of the terms in term_mask summed over sublattices, fp64 accumulation: -1/2 sum Ms V m.B for the terms
+ * bilinear in m (the energy densities of Eq.4, and Eq.6, in their discrete pair form), -sum Ms V m.B for
+ * the Zeeman term, -1/4 sum Ms V m.B for the quartic cubic anisotropy. */
 int mmx_energy(mmx_world* w, unsigned term_mask, double* joule_out);
 /* (1/2 sum sigma:eps V, 1/2 sum rho v^2 V) */
 int mmx_elastic_energy(mmx_world* w, double* strain_energy, double* kinetic_energy);
-/* max over cells and sublattices of |tau| (1/s). */
+/* max over cells and sublattices of |tau| (1/s): the measure of "relaxed". */
 int mmx_max_torque(mmx_world* w, double* out);
 
 /* Field of the magnet in a probe layer above it ("we calculate the out-of-plane component of the magnet's stray
